@@ -1,0 +1,162 @@
+/*
+ * include/pt_b200.h -- C ABI of the B200-native replica-exchange (parallel tempering)
+ * Metropolis Monte Carlo for an elastic bead-spring homopolymer.
+ *
+ * Method: Gross, Janke, Bachmann, "Massively parallelized replica-exchange simulations of
+ * polymers on GPUs", arxiv 1107.3490.  Line numbers below are those of PAPER.md.
+ *
+ *   model        E_LJ^mod + E_FENE, Eq. (1)-(4)                      PAPER.md:73-91  (Section 3.1)
+ *   update       single-monomer displacement + Metropolis, Eq. (5)   PAPER.md:93-101 (Section 3.2)
+ *   exchange     neighbouring temperatures, Eq. (6)                  PAPER.md:103-109 (Section 3.3)
+ *   measurement  once per sweep: energy, R_ee, R_gyr (Eq. 8)
+ *
+ * Conventions that hold for every call
+ *   - plain C, no torch types.  The handle is opaque.  Nothing throws or aborts across the ABI.
+ *   - every function returns an int status: PT_OK (0) or a negative PT_E* code;
+ *     pt_last_error(h) gives a NUL-terminated message owned by the library
+ *     (h == NULL: the message of the last failed pt_create* on this thread).
+ *   - pointers marked HOST are host memory, DEVICE are CUDA device memory on the current device.
+ *     Input arrays are caller-owned and are consumed (copied) before the call returns.
+ *     Output arrays are caller-allocated; NULL for an output means "skip it".
+ *   - everything returned is indexed by TEMPERATURE index i (0 = first entry of `temperatures`),
+ *     never by storage slot: the device swaps temperature labels, not coordinates,
+ *     which is equivalent to the exchange of conformations of PAPER.md:105.
+ *   - all work is enqueued on the cudaStream_t given at creation; pt_read / pt_recompute_energy
+ *     / pt_init synchronise that stream before they return, the others are asynchronous.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns PT_ECUDA.
+ *
+ * Random stream (all calls): Philox4x32-10, key = the ensemble's 64-bit seed (lo, hi),
+ *   counter = (a, b, ensemble, tag << 24 | temperature index):
+ *     tag 0 MOVE: a = step k within the sweep (0..N-1), b = sweep index t since pt_init;
+ *                 words -> (s_x, s_y, s_z, u_accept)
+ *     tag 1 PICK: same (a, b), only with PT_RANDOM_PICK: monomer = (w0 * N) >> 32
+ *     tag 2 SWAP: a = lower temperature index of the pair, b = exchange event index x,
+ *                 temperature field 0; w0 -> u_swap
+ *   word -> number, fp64:  s = (2w + 1 - 2^32) / 2^32 in (-1,1);  u = (w + 1/2) / 2^32 in (0,1)
+ *                   fp32:  s = (2 (w >> 8) + 1 - 2^24) / 2^24;     u = ((w >> 9) + 1/2) / 2^23
+ */
+#ifndef PT_B200_H
+#define PT_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pt_handle pt_handle;
+
+enum { PT_F64 = 0, PT_F32 = 1 };
+enum { PT_SEQUENTIAL = 0, PT_RANDOM_PICK = 1 };
+
+enum {
+  PT_OK = 0,
+  PT_EINVAL = -1, /* bad parameter (N < 2, M < 1, E < 1, M >= 2^24, non-positive or non-finite T or
+                     width, nbins < 0, emin >= emax, R <= 0, unknown flag, NULL required pointer,
+                     workspace too small or misaligned) */
+  PT_ESTATE = -2, /* sweeps / exchange / read before a successful pt_init */
+  PT_EBOND = -3,  /* a supplied conformation has a non-finite energy: a non-finite coordinate or a
+                     bond with |r - r0| >= R (FENE "diverges for r -> r0 +- R") */
+  PT_ENOMEM = -4,
+  PT_ECUDA = -5,  /* any CUDA error; the message carries cudaGetErrorString */
+  PT_ERANGE = -6  /* sweep counter t or event counter x would leave 32 bits (Philox counter words) */
+};
+
+typedef struct {
+  int32_t N;           /* monomers per chain, >= 2                                                    */
+  int32_t M;           /* replicas = temperatures per ensemble, 1 <= M < 2^24                         */
+  int32_t E;           /* independent ensembles, >= 1 (the throughput batch has 64)                   */
+  int32_t precision;   /* PT_F64: the reference path.  PT_F32: coordinates and pair arithmetic in
+                          fp32 (the paper's precision); E_run and moments stay fp64   */
+  int32_t select_mode; /* PT_SEQUENTIAL: step k moves monomer k.  PT_RANDOM_PICK: "a random monomer
+                          of the chain is picked"                                       */
+  int32_t nbins;       /* interior energy-histogram bins per temperature, 0 = no histogram            */
+  int32_t observables; /* != 0: accumulate R_ee^2 and R_gyr^2 (Eq. 8) once per sweep                  */
+  int32_t lanes;       /* threads that share one chain's Delta-E sum: 0 = choose from N and the chain
+                          count; 4, 8, 16, 32 = that many lanes of a warp; 64, 128, 256 = one CTA of
+                          that many threads per replica                                               */
+  double hist_emin, hist_emax;          /* histogram range, emin < emax (ignored if nbins == 0)       */
+  double eps, r0, R, K, rc_over_sigma;  /* model constants; the paper's are 1, 0.7, 0.3, 40, 2.5
+                                           (PAPER.md:81, :85); sigma = r0 / 2^(1/6) is derived        */
+} pt_params;
+
+/* Bytes of device memory a simulation with these parameters needs (0 if p is invalid). */
+uint64_t pt_workspace_bytes(const pt_params* p);
+
+/* Creates a simulation.  temperatures[M] HOST, > 0, k_B = 1, shared by all ensembles;
+ * move_halfwidths[M] HOST, > 0: half-width of the uniform displacement cube at each temperature
+ * (the paper's is 0.01 at every T).  cuda_stream: a cudaStream_t, or NULL for the
+ * default stream.  pt_create allocates its device memory with cudaMalloc; the _with_workspace
+ * form uses `device_ws` DEVICE (256-byte aligned, >= pt_workspace_bytes(p), owned by the caller
+ * and kept alive until pt_destroy) -- this is how the Python binding hands in torch memory. */
+int pt_create(pt_handle** out, const pt_params* p, const double* temperatures,
+              const double* move_halfwidths, void* cuda_stream);
+int pt_create_with_workspace(pt_handle** out, const pt_params* p, const double* temperatures,
+                             const double* move_halfwidths, void* cuda_stream, void* device_ws,
+                             uint64_t ws_bytes);
+int pt_destroy(pt_handle* h);
+
+/* seeds[E] HOST: one Philox key per ensemble.  conformations[E][M][N][3] HOST, fp64, the
+ * conformation that starts at temperature i of ensemble e (required).  Computes the running
+ * energy of every chain by the full O(N^2) sum of Eq. (4), zeroes all statistics, sets the sweep
+ * counter t = 0, the exchange-event counter x = 0 and the identity label permutation.
+ * PT_EBOND if any chain's energy is not finite (state stays uninitialised). */
+int pt_init(pt_handle* h, const uint64_t* seeds, const double* conformations);
+
+/* n >= 0 sweeps of every chain, no exchange.  One sweep = N attempted single-monomer moves
+ * (Section 3.2, Eq. 5), then one measurement: histogram, sum E, sum E^2, observables. */
+int pt_sweeps(pt_handle* h, int64_t n);
+
+/* One exchange event in every ensemble (Section 3.3, Eq. 6).  Event x tries the disjoint pairs
+ * (i, i+1) with i = x mod 2, x mod 2 + 2, ...; accept iff Delta = (beta_i - beta_{i+1})(E_i -
+ * E_{i+1}) >= 0 or u_swap < exp(Delta).  Swaps temperature labels on the device. */
+int pt_exchange(pt_handle* h);
+
+/* Repeats { pt_sweeps(exchange_every); pt_exchange() } until n_sweeps sweeps are done, without
+ * host round trips; a last partial block of sweeps is not followed by an exchange.
+ * exchange_every <= 0: no exchange at all. */
+int pt_run(pt_handle* h, int64_t n_sweeps, int64_t exchange_every);
+
+/* Synchronises the stream and copies results to HOST arrays (NULL = skip). */
+int pt_read(pt_handle* h,
+            double*   energies      /* [E][M]           running energy at temperature i              */,
+            uint64_t* histograms    /* [E][M][nbins+2]  interior bins, then underflow, overflow      */,
+            double*   moments       /* [E][M][3]        n_meas, sum E, sum E^2                       */,
+            uint64_t* move_counts   /* [E][M][3]        attempts, accepts, bond-range rejections     */,
+            uint64_t* swap_counts   /* [E][M-1][2]      attempts, accepts of pair (i, i+1)           */,
+            double*   conformations /* [E][M][N][3]     conformation currently at temperature i      */,
+            double*   obs_moments   /* [E][M][4]        sum Ree^2, sum Rg^2, sum Rg^4, sum Ree^4     */);
+
+/* Full O(N^2) recomputation of Eq. (4) for every chain, without touching the running energy:
+ * the invariant |E_run - E_full| is the caller's check.  energies_full[E][M] HOST. */
+int pt_recompute_energy(pt_handle* h, double* energies_full);
+
+/* Zeroes histograms, moments, observables and counters; keeps conformations, labels, t and x
+ * (discarding thermalisation). */
+int pt_reset_stats(pt_handle* h);
+
+/* Test support: per-decision trace written by the kernels, all DEVICE, temperature-indexed,
+ * NULL = off.  move_dec[E][M][cap_sweeps][N] one byte (0/1) per attempted move;
+ * swap_dec[E][cap_events][M-1] one byte per pair slot and event: 0 not attempted, 1 rejected,
+ * 2 accepted; e_trace[E][M][cap_sweeps] the running energy after every sweep.  Sweeps / events
+ * beyond the capacities are not recorded.  Buffers stay owned by the caller. */
+int pt_set_trace(pt_handle* h, int64_t cap_sweeps, int64_t cap_events, uint8_t* move_dec,
+                 uint8_t* swap_dec, double* e_trace);
+
+/* Sweep and exchange-event counters since pt_init. */
+int pt_counters(const pt_handle* h, int64_t* t_sweeps, int64_t* x_events);
+
+/* How the sweep kernel is mapped: lanes per chain (as in pt_params.lanes, resolved), chains per
+ * CTA, CTAs in the grid, dynamic shared memory bytes per CTA.  Any pointer may be NULL. */
+int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,
+                   int32_t* smem_bytes);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+int64_t pt_kernel_launches(const pt_handle* h);
+
+const char* pt_last_error(const pt_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

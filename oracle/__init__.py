@@ -34,7 +34,7 @@ def build(force: bool = False) -> Path:
 class OrcParams(C.Structure):
     _fields_ = [
         ("N", C.c_int32), ("M", C.c_int32), ("E", C.c_int32),
-        ("select_mode", C.c_int32), ("nbins", C.c_int32), ("pad_", C.c_int32),
+        ("select_mode", C.c_int32), ("nbins", C.c_int32), ("e_offset", C.c_int32),
         ("hist_emin", C.c_double), ("hist_emax", C.c_double),
         ("eps", C.c_double), ("r0", C.c_double), ("R", C.c_double), ("K", C.c_double),
         ("rc_over_sigma", C.c_double),
@@ -42,8 +42,8 @@ class OrcParams(C.Structure):
 
 
 def make_params(N, M=1, E=1, select_mode=0, nbins=0, hist_emin=0.0, hist_emax=1.0,
-                eps=1.0, r0=0.7, R=0.3, K=40.0, rc_over_sigma=2.5) -> OrcParams:
-    return OrcParams(N, M, E, select_mode, nbins, 0, hist_emin, hist_emax, eps, r0, R, K,
+                eps=1.0, r0=0.7, R=0.3, K=40.0, rc_over_sigma=2.5, e_offset=0) -> OrcParams:
+    return OrcParams(N, M, E, select_mode, nbins, e_offset, hist_emin, hist_emax, eps, r0, R, K,
                      rc_over_sigma)
 
 

@@ -202,7 +202,7 @@ struct orc_state {
 orc_state* orc_create(const orc_params* p, const double* temperatures, const double* widths)
 {
   if (!p || !temperatures || !widths) return NULL;
-  if (p->N < 2 || p->M < 1 || p->E < 1 || p->nbins < 0) return NULL;
+  if (p->N < 2 || p->M < 1 || p->E < 1 || p->nbins < 0 || p->e_offset < 0) return NULL;
   if (p->nbins > 0 && !(p->hist_emin < p->hist_emax)) return NULL;
   orc_state* s = (orc_state*)calloc(1, sizeof(orc_state));
   if (!s) return NULL;
@@ -285,12 +285,12 @@ static void sweep_chain(orc_state* s, int e, int i, int64_t t)
     /* "A random monomer of the chain is picked" -- or sequential order (reading R3) */
     int m = k;
     if (p->select_mode == 1) {
-      draw(s->seed[e], (uint32_t)k, (uint32_t)t, (uint32_t)e, TAG_PICK, (uint32_t)i, w);
+      draw(s->seed[e], (uint32_t)k, (uint32_t)t, (uint32_t)(p->e_offset + e), TAG_PICK, (uint32_t)i, w);
       m = (int)(((uint64_t)w[0] * (uint64_t)N) >> 32);
     }
     /* "a shift of its coordinates by a random vector ... components uniformly distributed"
      * in [-d, d] */
-    draw(s->seed[e], (uint32_t)k, (uint32_t)t, (uint32_t)e, TAG_MOVE, (uint32_t)i, w);
+    draw(s->seed[e], (uint32_t)k, (uint32_t)t, (uint32_t)(p->e_offset + e), TAG_MOVE, (uint32_t)i, w);
     double xnew[3];
     for (int a = 0; a < 3; ++a) {
       double delta = d * orc_word_to_sym(w[a]);   /* one rounding */
@@ -370,7 +370,7 @@ void orc_exchange(orc_state* s)
       size_t ci = (size_t)e * M + i, cj = ci + 1;
       double delta = (s->beta[i] - s->beta[i + 1]) * (s->Erun[ci] - s->Erun[cj]);
       uint32_t w[4];
-      draw(s->seed[e], (uint32_t)i, (uint32_t)s->x, (uint32_t)e, TAG_SWAP, 0u, w);
+      draw(s->seed[e], (uint32_t)i, (uint32_t)s->x, (uint32_t)(p->e_offset + e), TAG_SWAP, 0u, w);
       double u = orc_word_to_u01(w[0]);
       int accept = (delta >= 0.0) ? 1 : (u < exp(delta));
       uint64_t* sc = s->scount + ((size_t)e * (M - 1) + i) * 2;

@@ -35,7 +35,9 @@ typedef struct {
   int32_t E;           /* independent ensembles (>= 1)                               */
   int32_t select_mode; /* 0 = sequential monomer order, 1 = random pick */
   int32_t nbins;       /* interior histogram bins per temperature (0 = none)         */
-  int32_t pad_;
+  int32_t e_offset;    /* index of this state's ensemble 0 in the caller's job: the Philox counter
+                          word is e_offset + e, so that a sample of the ensembles of a large job
+                          can be recomputed one by one (0 = the whole job)                */
   double hist_emin, hist_emax;
   double eps, r0, R, K, rc_over_sigma;
 } orc_params;

@@ -1,0 +1,73 @@
+// Internal declarations shared by the translation units of libpt_b200.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "pt_b200.h"
+
+// Coordinates that can never be within the cutoff of a real monomer.  Used for the padding
+// entries of a chain's shared-memory arrays and to hide the moved monomer from its own sum.
+#define PT_FAR 1.0e6
+
+// Device-side view of one simulation; passed by value to every kernel.
+struct PtDev {
+  int N, M, E, C;        // C = E*M chains
+  int Ng;                // padded length of one coordinate array in HBM (even)
+  int nbins, select_mode, observables;
+  double hist_emin, hist_scale;  // scale = nbins / (emax - emin)
+  // model constants, host-computed in fp64
+  double ljA;    // 4 eps sigma^12
+  double ljB;    // 4 eps sigma^6
+  double ljC;    // E_LJ(r_c) = 4 eps [(sigma/r_c)^12 - (sigma/r_c)^6]
+  double rc2;    // r_c^2
+  double sigma2; // sigma^2
+  double eps4;   // 4 eps
+  double r0, R, invR;
+  double feneC;  // -(K/2) R^2
+  // state, slot-indexed: slot s = e*M + (slot within ensemble)
+  void* coords;          // Real [C][3][Ng]  SoA per chain: x[], y[], z[]
+  double* erun;          // [C]
+  int* temp_of_slot;     // [C] temperature index (within the ensemble) the slot currently has
+  int* slot_of_temp;     // [C] slot (within the ensemble) that currently has temperature i
+  // per-temperature constants and keys
+  const double* beta;    // [M]
+  const double* width;   // [M]
+  const uint2* keys;     // [E]
+  // statistics, temperature-indexed: ti = e*M + i
+  unsigned long long* hist;    // [C][nbins+2]
+  double* mom;                 // [C][3]
+  double* obs;                 // [C][4]
+  unsigned long long* mcount;  // [C][3]
+  unsigned long long* scount;  // [E][max(M-1,1)][2]
+  // trace (test support), temperature-indexed
+  unsigned char* tr_move;
+  unsigned char* tr_swap;
+  double* tr_e;
+  long long cap_sweeps, cap_events;
+};
+
+struct PtLaunch {
+  int lanes;           // resolved lanes per chain
+  int chains_per_cta;
+  int threads;         // per CTA
+  int grid;
+  int smem_bytes;      // dynamic shared memory per CTA
+  int sstride;         // shared-memory stride between chains, in Reals
+  int Ns;              // padded monomers per coordinate array in shared memory
+};
+
+// pt_sweep.cu
+cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan);
+cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& plan, uint32_t t0,
+                            int n_sweeps, cudaStream_t stream);
+
+// pt_aux.cu
+cudaError_t pt_launch_scatter_init(const PtDev& d, int precision, const double* staging,
+                                   cudaStream_t stream);
+cudaError_t pt_launch_zero_stats(const PtDev& d, cudaStream_t stream);
+cudaError_t pt_launch_full_energy(const PtDev& d, int precision, double* out_slot_energy,
+                                  cudaStream_t stream);
+cudaError_t pt_launch_exchange(const PtDev& d, uint32_t x, cudaStream_t stream);
+cudaError_t pt_launch_gather(const PtDev& d, int precision, const double* slot_energy,
+                             double* out_energy_by_temp, double* out_conf_by_temp,
+                             cudaStream_t stream);
