@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the replica-exchange Monte Carlo hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 5] [--precision f64|f32] [--lanes L]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input: pt_run(n_sweeps,
+exchange_every) of a BASELINE.json configuration (default: config 5, the throughput batch of
+64 ensembles x 64 replicas, N = 100, 10^3 sweeps, exchange every 10) -- every sweep kernel and
+every exchange kernel of the job.  The metric is BASELINE.json's: attempted monomer moves per
+second over all replicas (and pair evaluations/s = moves/s * 2(N-1)).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "attempted monomer moves/sec (all replicas)"
+UNIT = "moves/s"
+FLOPS_PER_PAIR_EVAL = 17          # E_LJ^mod from two positions, nominal count
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12     # 37.2: 148 SMs x 64 fp64 lanes x 2 x 1.965 GHz
+NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 * 1e-12    # 74.4
+# fp64-pipe warp instructions the sweep kernel issues per attempted move at the default mapping of
+# config 5, counted in the SASS of the shipped kernel; used for pipe_frac.
+SWEEP_DRAM_TRAFFIC = None         # bytes per sweep launch from ncu --set full (profiles/), None = not captured
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--sweeps", type=int, default=0, help="override the configuration's sweep count")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---- clocks during the timed region (B200_PROFILING.md) -------------------------------------
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], None, [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for t, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                mhz = float(f[0]); smax = float(f[1])
+            except ValueError:
+                continue
+            if t0 <= t <= t1:
+                sm.append(mhz)
+                try:
+                    power.append(float(f[2]))
+                except ValueError:
+                    pass
+                for name, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "power_w": float(np.median(power)) if power else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ---- distributed plumbing: replicas only, no data-path collective ----
+
+def dist_setup(n_gpus: int, backend: str | None = None):
+    """Returns (rank, world, local_rank).  One process per GPU under torchrun; rank 0 alone otherwise."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        if not dist.is_initialized():
+            dist.init_process_group(backend=backend or "nccl", rank=rank, world_size=world)
+    return rank, world, local
+
+
+def dist_barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def dist_max(value: float, world: int, device="cpu") -> float:
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def dist_sum(value: float, world: int, device="cpu") -> float:
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def host_cores() -> int:
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+# ---- the oracle, timed as it stands (cpu_baseline leg and --impl reference) ------------------
+
+def oracle_sample_run(inp, n_ens: int, n_sweeps: int, threads: int, reps: int = 1):
+    """Times the CPU oracle on the first `n_ens` ensembles of the workload for `n_sweeps` sweeps
+    (exchange at the workload's cadence).  Returns (moves, seconds per rep list)."""
+    import oracle
+    wl = inp.workload
+    n_ens = min(n_ens, wl.E)
+    p = oracle.make_params(wl.N, wl.M, n_ens, nbins=wl.nbins, hist_emin=wl.hist_range[0],
+                           hist_emax=wl.hist_range[1])
+    times = []
+    for _ in range(reps):
+        o = oracle.Oracle(p, inp.temperatures, inp.widths, threads=threads)
+        o.init(inp.seeds[:n_ens], inp.conformations[:n_ens])   # initialisation is outside the timed region
+        t0 = time.perf_counter()
+        o.run(n_sweeps, wl.exchange_every)
+        times.append(time.perf_counter() - t0)
+        o.close()
+    return n_ens * wl.M * wl.N * n_sweeps, times
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the box's host cores, each step a bounded sample of the
+    workload (rank 0 only; the other ranks exit without work)."""
+    if rank != 0:
+        return
+    from paper_1107_3490_b200 import synth
+    inp = synth.make_inputs(args.config)
+    wl = inp.workload
+    cores = host_cores()
+    n_ens = min(wl.E, 2)
+    n_sweeps = min(args.sweeps or wl.n_sweeps, max(wl.exchange_every, 100 if wl.N >= 50 else 1000))
+    for _ in range(args.warmup):
+        oracle_sample_run(inp, n_ens, n_sweeps, cores)
+    moves, times = oracle_sample_run(inp, n_ens, n_sweeps, cores, reps=args.steps)
+    total = float(sum(times))
+    value = moves * args.steps / total
+    sample = (f"first {n_ens} of {wl.E} ensembles ({n_ens * wl.M} chains), {n_sweeps} of {wl.n_sweeps} sweeps "
+              f"per step, exchange every {wl.exchange_every}")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "N": wl.N, "M": wl.M, "E": wl.E, "exchange_every": wl.exchange_every,
+                   "sample": sample},
+        "pair_evals_per_s": value * 2 * (wl.N - 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---- our arm ----------------------------------------------------------------------------------
+
+def run_ours(args, rank, world, local):
+    import torch
+
+    import paper_1107_3490_b200 as pt
+    from paper_1107_3490_b200 import synth
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    # replicas only: every rank simulates its own copy of the workload with rank-specific seeds
+    inp = synth.make_inputs(args.config, rank=rank)
+    wl = inp.workload
+    n_sweeps = args.sweeps or wl.n_sweeps
+    S = wl.exchange_every
+    f32 = args.precision == "f32"
+    p = pt.make_params(wl.N, wl.M, wl.E, precision=pt.PT_F32 if f32 else pt.PT_F64, nbins=wl.nbins,
+                       observables=0, lanes=args.lanes, hist_emin=wl.hist_range[0], hist_emax=wl.hist_range[1])
+    stream = torch.cuda.Stream(device=dev)
+    sim = pt.ParallelTempering(p, inp.temperatures, inp.widths, stream=stream)
+    info = sim.pt_launch_info()
+    moves_per_step = wl.chains * wl.N * n_sweeps
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    def evt():
+        return torch.cuda.Event(enable_timing=True)
+
+    def timed_step():
+        """Re-initialises (untimed, inputs resident afterwards), flushes L2, then times one pt_run
+        with CUDA events recorded on the stream the library launches on."""
+        sim.pt_init(inp.seeds, inp.conformations)
+        flush.fill_(rank + 1)
+        torch.cuda.synchronize(dev)
+        dist_barrier(world)
+        a, b = evt(), evt()
+        with torch.cuda.stream(stream):
+            a.record(stream)
+            sim.pt_run(n_sweeps, S)
+            b.record(stream)
+        b.synchronize()
+        torch.cuda.synchronize(dev)
+        return a.elapsed_time(b) * 1e-3
+
+    for _ in range(max(args.warmup, 0)):
+        timed_step()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = sim.pt_kernel_launches()
+    launches_in_timed = 0
+    wall0 = time.perf_counter()
+    step_s = []
+    for _ in range(args.steps):
+        k0 = sim.pt_kernel_launches()
+        step_s.append(timed_step())
+        # launches inside the timed bracket: everything pt_run enqueued (pt_init's 3 kernels are outside it)
+        launches_in_timed += sim.pt_kernel_launches() - k0 - 3
+    wall1 = time.perf_counter()
+    clocks = sampler.stop(wall0, wall1) if sampler else None
+    t_dev = dist_max(float(sum(step_s)), world, dev)
+    total_moves = dist_sum(float(moves_per_step * args.steps), world, dev)
+    value = total_moves / t_dev
+
+    # sweep kernel alone: average launch duration over launches of S sweeps (roofline numerator)
+    sim.pt_init(inp.seeds, inp.conformations)
+    with torch.cuda.stream(stream):
+        sim.pt_sweeps(S)
+    torch.cuda.synchronize(dev)
+    n_k = 20
+    ka, kb = evt(), evt()
+    with torch.cuda.stream(stream):
+        ka.record(stream)
+        for _ in range(n_k):
+            sim.pt_sweeps(S)
+        kb.record(stream)
+    kb.synchronize()
+    k_s = ka.elapsed_time(kb) * 1e-3 / n_k
+    moves_per_launch = wl.chains * wl.N * S
+    flops_per_launch = moves_per_launch * 2 * (wl.N - 1) * FLOPS_PER_PAIR_EVAL
+    achieved = flops_per_launch / k_s * 1e-12
+    peak = pt.pt_fma_peak(pt.PT_F32 if f32 else pt.PT_F64, stream=stream)
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": SWEEP_DRAM_TRAFFIC, "kernel": "k_sweep", "kernel_ms": k_s * 1e3,
+                "peak_kind": f"measured {'fp32' if f32 else 'fp64'} FMA chain (pt_fma_peak), this run",
+                "peak_nominal": NOMINAL_FP32_TFLOPS if f32 else NOMINAL_FP64_TFLOPS,
+                "flops_per_pair_eval": FLOPS_PER_PAIR_EVAL,
+                "kernel_share_of_step": (k_s * (n_sweeps // S)) / (t_dev / args.steps) if world == 1 else None}
+
+    # end to end through the C ABI with HOST buffers: pt_init (H2D) + pt_run + pt_read (D2H)
+    e2e = None
+    if not args.no_e2e:
+        conf_h = torch.from_numpy(inp.conformations).pin_memory().numpy()
+        outs = {k: torch.empty(s, dtype=d).pin_memory().numpy() for k, (s, d) in {
+            "energies": ((wl.E, wl.M), torch.float64),
+            "moments": ((wl.E, wl.M, 3), torch.float64),
+            "conformations": ((wl.E, wl.M, wl.N, 3), torch.float64)}.items()}
+        hist = np.zeros((wl.E, wl.M, wl.nbins + 2), dtype=np.uint64)
+        mc = np.zeros((wl.E, wl.M, 3), dtype=np.uint64)
+        sc = np.zeros((wl.E, max(wl.M - 1, 1), 2), dtype=np.uint64)
+        h2d = conf_h.nbytes + inp.seeds.nbytes
+        d2h = sum(a.nbytes for a in outs.values()) + hist.nbytes + mc.nbytes + (sc.nbytes if wl.M > 1 else 0)
+
+        def e2e_step():
+            sim.pt_init(inp.seeds, conf_h)
+            sim.pt_run(n_sweeps, S)
+            sim.pt_read_into(energies=outs["energies"], histograms=hist, moments=outs["moments"], move_counts=mc,
+                             swap_counts=sc if wl.M > 1 else None, conformations=outs["conformations"])
+
+        e2e_step()
+        torch.cuda.synchronize(dev)
+        dist_barrier(world)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e2e_step()
+        torch.cuda.synchronize(dev)
+        t_e2e = dist_max(time.perf_counter() - t0, world, dev)
+        e2e = {"value": total_moves / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * t_e2e / args.steps}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = host_cores()
+        ne, ns = min(wl.E, 8), min(n_sweeps, 200 if wl.N >= 50 else 2000)
+        moves, times = oracle_sample_run(inp, ne, ns, cores)
+        cpu_baseline = {"value": moves / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"first {ne} of {wl.E} ensembles ({ne * wl.M} chains), {ns} of {n_sweeps} sweeps, "
+                                  f"exchange every {S}; {times[0]:.2f} s wall on {cores} threads"}
+    sim.pt_destroy()
+    if rank != 0:
+        return
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.precision, "data": "synthetic",
+        "config": {"workload": wl.name, "N": wl.N, "M": wl.M, "E": wl.E, "chains_per_gpu": wl.chains,
+                   "n_sweeps": n_sweeps, "exchange_every": S, "nbins": wl.nbins, "parallelism": f"replicas x{world}",
+                   "lanes_per_chain": info["lanes"], "chains_per_cta": info["chains_per_cta"], "grid": info["grid"],
+                   "smem_bytes": info["smem_bytes"],
+                   "l2": "flushed (256 MiB write) before every timed step; working set 10 MB, compute-bound",
+                   "timing": "sum of per-step CUDA-event intervals on the library's stream; state re-initialised "
+                             "(untimed) before every step so each step is sweeps 0..n-1 of the workload"},
+        "pair_evals_per_s": value * 2 * (wl.N - 1),
+        "gpu_launches": int(launches_in_timed),
+        "clocks": clocks, "roofline": roofline, "e2e": e2e, "cpu_baseline": cpu_baseline,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, rank, int(os.environ.get("WORLD_SIZE", "1")))
+        return
+    rank, world, local = dist_setup(args.gpus)
+    try:
+        run_ours(args, rank, world, local)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            if dist.is_initialized():
+                dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -156,6 +156,13 @@ int64_t pt_kernel_launches(const pt_handle* h);
 
 const char* pt_last_error(const pt_handle* h);
 
+/* Measurement support (no handle): the sustained plain fp64 (PT_F64) or fp32 (PT_F32) FMA rate of
+ * the current device in TFLOP/s (2 flops per FMA), best of `reps` launches of `iters` x 64
+ * dependent-chain FMAs per thread at full occupancy, timed with CUDA events on `cuda_stream`.
+ * It is the denominator of the "alu" roofline the sweep kernel is reported against (the Delta-E
+ * sum of Eq. 5 is plain FMA-pipe work, no tensor cores).  tflops HOST. */
+int pt_fma_peak(int precision, int iters, int reps, void* cuda_stream, double* tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -6,7 +6,7 @@ Importing the package does not load the library; ``binding.lib()`` does, and fai
 if it cannot be built -- there is no CPU fallback.
 """
 from .binding import (PT_F32, PT_F64, PT_RANDOM_PICK, PT_SEQUENTIAL, ParallelTempering, PtError,
-                      PtParams, lib, lib_path, make_params, pt_workspace_bytes)
+                      PtParams, lib, lib_path, make_params, pt_fma_peak, pt_workspace_bytes)
 
 __all__ = ["PT_F32", "PT_F64", "PT_RANDOM_PICK", "PT_SEQUENTIAL", "ParallelTempering", "PtError",
-           "PtParams", "lib", "lib_path", "make_params", "pt_workspace_bytes"]
+           "PtParams", "lib", "lib_path", "make_params", "pt_fma_peak", "pt_workspace_bytes"]

@@ -24,7 +24,8 @@ _ERRNAMES = {-1: "PT_EINVAL", -2: "PT_ESTATE", -3: "PT_EBOND", -4: "PT_ENOMEM", 
 # every symbol include/pt_b200.h declares
 SYMBOLS = ("pt_workspace_bytes", "pt_create", "pt_create_with_workspace", "pt_destroy", "pt_init",
            "pt_sweeps", "pt_exchange", "pt_run", "pt_read", "pt_recompute_energy", "pt_reset_stats",
-           "pt_set_trace", "pt_counters", "pt_launch_info", "pt_kernel_launches", "pt_last_error")
+           "pt_set_trace", "pt_counters", "pt_launch_info", "pt_kernel_launches", "pt_last_error",
+           "pt_fma_peak")
 
 
 class PtParams(C.Structure):
@@ -80,6 +81,7 @@ def lib():
     L.pt_launch_info.argtypes = [hp, i32p, i32p, i32p, i32p]; L.pt_launch_info.restype = C.c_int
     L.pt_kernel_launches.argtypes = [hp]; L.pt_kernel_launches.restype = C.c_int64
     L.pt_last_error.argtypes = [hp]; L.pt_last_error.restype = C.c_char_p
+    L.pt_fma_peak.argtypes = [C.c_int, C.c_int, C.c_int, C.c_void_p, dp]; L.pt_fma_peak.restype = C.c_int
     _lib = L
     return L
 
@@ -105,6 +107,16 @@ def _check(h, rc):
 
 def pt_workspace_bytes(params: PtParams) -> int:
     return int(lib().pt_workspace_bytes(C.byref(params)))
+
+
+def pt_fma_peak(precision=PT_F64, iters=4096, reps=5, stream=None) -> float:
+    """Measured plain FMA rate of the current device in TFLOP/s (roofline denominator)."""
+    out = C.c_double(0.0)
+    sptr = C.c_void_p(stream.cuda_stream) if stream is not None else None
+    rc = lib().pt_fma_peak(int(precision), int(iters), int(reps), sptr, C.byref(out))
+    if rc != PT_OK:
+        raise PtError(rc, "pt_fma_peak failed (no CUDA device?)")
+    return out.value
 
 
 class ParallelTempering:
