@@ -73,7 +73,7 @@ typedef struct {
   int32_t nbins;       /* interior energy-histogram bins per temperature, 0 = no histogram            */
   int32_t observables; /* != 0: accumulate R_ee^2 and R_gyr^2 (Eq. 8) once per sweep                  */
   int32_t lanes;       /* threads that share one chain's Delta-E sum: 0 = choose from N and the chain
-                          count; 4, 8, 16, 32 = that many lanes of a warp; 64, 128, 256 = one CTA of
+                          count; 8, 16, 32 = that many lanes of a warp; 64, 128, 256 = one CTA of
                           that many threads per replica                                               */
   double hist_emin, hist_emax;          /* histogram range, emin < emax (ignored if nbins == 0)       */
   double eps, r0, R, K, rc_over_sigma;  /* model constants; the paper's are 1, 0.7, 0.3, 40, 2.5

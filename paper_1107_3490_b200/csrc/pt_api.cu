@@ -65,8 +65,8 @@ bool params_ok(const pt_params* p, std::string* why)
   if (p->nbins > 0 && !(p->hist_emin < p->hist_emax && isfinite(p->hist_emin) && isfinite(p->hist_emax))) {
     *why = "histogram range must satisfy emin < emax"; return false;
   }
-  switch (p->lanes) { case 0: case 4: case 8: case 16: case 32: case 64: case 128: case 256: break;
-    default: *why = "lanes must be 0, 4, 8, 16, 32, 64, 128 or 256"; return false; }
+  switch (p->lanes) { case 0: case 8: case 16: case 32: case 64: case 128: case 256: break;
+    default: *why = "lanes must be 0, 8, 16, 32, 64, 128 or 256"; return false; }
   if (!(p->eps > 0.0) || !isfinite(p->eps)) { *why = "eps must be > 0"; return false; }
   if (!(p->r0 > 0.0) || !isfinite(p->r0)) { *why = "r0 must be > 0"; return false; }
   if (!(p->R > 0.0) || !isfinite(p->R)) { *why = "R must be > 0"; return false; }

@@ -32,7 +32,8 @@ __device__ __forceinline__ uint4 pt_draw(uint2 key, uint32_t a, uint32_t b, uint
   return pt_philox4x32_10(make_uint4(a, b, e, (tag << 24) | i), key);
 }
 
-// ---- word -> number.  Every value is exactly representable, so the proposal is bit-reproducible.
+// ---- word -> number, proposal, reciprocal, cutoff test, per precision.
+// Every random value is exactly representable, so the proposal is bit-reproducible.
 template <typename Real> struct PtNum;
 
 template <> struct PtNum<double> {
@@ -51,18 +52,41 @@ template <> struct PtNum<double> {
   {
     return __dadd_rn(x, __dmul_rn(d, s));
   }
+  // 1/d for finite d > 0: MUFU.RCP64H seed (relative error < 2^-19.9 measured on B200) and one
+  // cubic Newton step x (1 + e + e^2), e = 1 - d x  ->  relative error e^3 < 2^-59 before the
+  // final rounding; measured worst case 2 ulp.  3 fp64-pipe instructions instead of the ~9 of an
+  // IEEE division.  d = 0 gives +inf, d = inf gives NaN (callers mask such pairs out).
   static __device__ __forceinline__ double rcp(double d)
   {
-    // MUFU.RCP64H seed, then one cubic Newton step: x (1 + e + e^2), e = 1 - d x.
     double x;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
     const double e = fma(-d, x, 1.0);
-    const double p = fma(e, e, e);
-    const double y = fma(x, p, x);
-    // second (quadratic) correction keeps the result within ~1 ulp whatever the seed quality
-    const double e2 = fma(-d, y, 1.0);
-    return fma(y, e2, y);
+    return fma(x, fma(e, e, e), x);
   }
+  // r2 < rc2 for r2 >= 0 (or NaN), decided on the integer pipe: the bit patterns of non-negative
+  // doubles are ordered like the numbers; NaN and anything with the sign bit set compare false.
+  static __device__ __forceinline__ bool below(double r2, double rc2)
+  {
+    return (unsigned long long)__double_as_longlong(r2) < (unsigned long long)__double_as_longlong(rc2);
+  }
+  // v if keep, else a huge finite number (> 4e307 whatever the low word): beyond every cutoff, and
+  // still finite after the few additions that follow.  One integer select on the high word.
+  static __device__ __forceinline__ double keep_or_far(double v, bool keep)
+  {
+    return __hiloint2double(keep ? __double2hiint(v) : 0x7fe00000, __double2loint(v));
+  }
+  // inside ? 1/d : 0 -- the mask is applied to the seed (one integer select on its high word; a
+  // zero seed stays zero through the Newton step), so that the sums need no select afterwards.
+  static __device__ __forceinline__ double rcp_masked(double d, bool inside)
+  {
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    x = __hiloint2double(inside ? __double2hiint(x) : 0, __double2loint(x));
+    const double e = fma(-d, x, 1.0);
+    return fma(x, fma(e, e, e), x);
+  }
+  static __device__ __forceinline__ double sqrt_(double v) { return sqrt(v); }
+  static __device__ __forceinline__ double log_(double v) { return log(v); }
 };
 
 template <> struct PtNum<float> {
@@ -84,22 +108,67 @@ template <> struct PtNum<float> {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return x;
   }
+  static __device__ __forceinline__ bool below(float r2, float rc2) { return r2 < rc2; }
+  static __device__ __forceinline__ float keep_or_far(float v, bool keep)
+  {
+    return keep ? v : __int_as_float(0x7f000000);
+  }
+  static __device__ __forceinline__ float rcp_masked(float d, bool inside)
+  {
+    float x;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
+    return inside ? x : 0.0f;
+  }
+  static __device__ __forceinline__ float sqrt_(float v) { return sqrtf(v); }
+  // the paper's fp32 kernels use the fast-math intrinsics (__logf)
+  static __device__ __forceinline__ float log_(float v) { return __logf(v); }
 };
 
 // ---- Eq. (1)-(2) as a function of r^2:
 //   E_LJ^mod = 4 eps [(sigma/r)^12 - (sigma/r)^6] - E_LJ(r_c)  for r < r_c,  0 otherwise
 //            = u (A u - B) - C,   u = 1/r^6,  A = 4 eps sigma^12,  B = 4 eps sigma^6,  C = E_LJ(r_c)
-// The caller applies the r < r_c selection.
+// The sums accumulate u (A u - B) with u = 0 for the pairs outside the cutoff, and count the pairs
+// inside; the caller subtracts C * count once per sum.
 template <typename Real> struct PtLJ {
-  Real A, B, C, rc2;
+  Real A, nB, C, rc2;
   __device__ __forceinline__ explicit PtLJ(const PtDev& d)
-      : A((Real)d.ljA), B((Real)d.ljB), C((Real)d.ljC), rc2((Real)d.rc2)
+      : A((Real)d.ljA), nB((Real)-d.ljB), C((Real)d.ljC), rc2((Real)d.rc2)
   {
   }
-  __device__ __forceinline__ Real inside(Real r2) const
+  // acc += u (A u - B) for one squared distance; returns whether it lies inside the cutoff
+  __device__ __forceinline__ bool add(Real r2, Real& acc) const
   {
-    const Real inv = PtNum<Real>::rcp(r2);
+    const bool inside = PtNum<Real>::below(r2, rc2);
+    const Real inv = PtNum<Real>::rcp_masked(r2, inside);
     const Real u = inv * inv * inv;
-    return fma(u, fma(A, u, -B), -C);
+    acc = fma(u, fma(A, u, nB), acc);
+    return inside;
+  }
+};
+
+template <typename Real> struct PtVec2;
+template <> struct PtVec2<double> { typedef double2 type; };
+template <> struct PtVec2<float> { typedef float2 type; };
+
+// One chain's coordinates in shared memory: (x, y) pairs in one array, z in another, so that a
+// partner costs one 128-bit and one 64-bit load (fp64) with consecutive lanes on consecutive banks.
+template <typename Real> struct PtCoords {
+  typename PtVec2<Real>::type* xy;
+  Real* z;
+  __device__ __forceinline__ PtCoords(Real* base, int Ns)
+      : xy(reinterpret_cast<typename PtVec2<Real>::type*>(base)), z(base + 2 * (size_t)Ns)
+  {
+  }
+  __device__ __forceinline__ void get(int j, Real& x, Real& y, Real& zz) const
+  {
+    const typename PtVec2<Real>::type v = xy[j];
+    x = v.x; y = v.y; zz = z[j];
+  }
+  __device__ __forceinline__ void set(int j, Real x, Real y, Real zz) const
+  {
+    typename PtVec2<Real>::type v;
+    v.x = x; v.y = y;
+    xy[j] = v;
+    z[j] = zz;
   }
 };

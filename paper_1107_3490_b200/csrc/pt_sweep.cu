@@ -15,37 +15,6 @@
 
 namespace {
 
-template <typename Real> struct Fene;
-template <> struct Fene<double> {
-  // Eq. (3): -(K/2) R^2 log[1 - ((r - r0)/R)^2]; +inf outside (r0-R, r0+R)
-  static __device__ __forceinline__ double eval(const PtDev& d, double r2, bool* inside)
-  {
-    const double r = sqrt(r2);
-    const double q = (r - d.r0) * d.invR;
-    const double g = fma(-q, q, 1.0);
-    *inside = (g > 0.0);
-    return *inside ? d.feneC * log(g) : __longlong_as_double(0x7ff0000000000000ll);
-  }
-  static __device__ __forceinline__ bool metropolis(double u, double beta, double dE)
-  {
-    return u < exp(-beta * dE);
-  }
-};
-template <> struct Fene<float> {
-  static __device__ __forceinline__ float eval(const PtDev& d, float r2, bool* inside)
-  {
-    const float r = sqrtf(r2);
-    const float q = (r - (float)d.r0) * (float)d.invR;
-    const float g = fmaf(-q, q, 1.0f);
-    *inside = (g > 0.0f);
-    return *inside ? (float)d.feneC * logf(g) : __int_as_float(0x7f800000);
-  }
-  static __device__ __forceinline__ bool metropolis(float u, double beta, float dE)
-  {
-    return u < expf(-(float)beta * dE);
-  }
-};
-
 template <typename Real, int L> __device__ __forceinline__ Real group_sum(Real v)
 {
 #pragma unroll
@@ -94,7 +63,8 @@ __device__ __forceinline__ void measure_energy(const PtDev& d, ChainCtx& c, uint
     if (b >= 0.0 && b < (double)d.nbins) idx = (int)b;
     else if (b < 0.0) idx = d.nbins;       // underflow
     else idx = d.nbins + 1;                // overflow (and NaN)
-    atomicAdd(d.hist + (size_t)c.ti * (size_t)(d.nbins + 2) + idx, 1ull);
+    // temperature index ti is owned by exactly one chain during a launch: no atomic needed
+    d.hist[(size_t)c.ti * (size_t)(d.nbins + 2) + idx] += 1ull;
   }
   c.mom1 = __dadd_rn(c.mom1, E);
   c.mom2 = __dadd_rn(c.mom2, __dmul_rn(E, E));
@@ -118,111 +88,187 @@ __device__ __forceinline__ void ctx_store(const PtDev& d, const ChainCtx& c, int
   d.mcount[3 * c.ti + 2] += c.brej;
 }
 
+// The proposal of one step (A2): which monomer, where to, and the acceptance uniform.
+template <typename Real> struct Proposal {
+  int m;
+  Real sx, sy, sz, u;
+};
+
+template <typename Real>
+__device__ __forceinline__ Proposal<Real> draw_proposal(const ChainCtx& c, bool pick, int N, uint32_t k, uint32_t t)
+{
+  Proposal<Real> p;
+  p.m = (int)k;
+  if (pick) {   // "a random monomer of the chain is picked"
+    const uint4 wp = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
+    p.m = (int)__umulhi(wp.x, (uint32_t)N);
+  }
+  const uint4 w = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
+  p.sx = PtNum<Real>::sym(w.x);
+  p.sy = PtNum<Real>::sym(w.y);
+  p.sz = PtNum<Real>::sym(w.z);
+  p.u = PtNum<Real>::u01(w.w);
+  return p;
+}
+
+// A3 for one partner j (other = "j is not the moved monomer"): adds u (A u - B) of the new and of
+// the old distance to en / eo when inside the cutoff and counts the inside pairs (cnt = #new - #old)
+// for the shift -C.  The new squared distance follows from the old one:
+// |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2 with b = x_m - x_j.  Branch-free: the moved monomer
+// itself is pushed to a huge distance, pairs outside the cutoff contribute u = 0.
+template <typename Real>
+__device__ __forceinline__ void pair_terms(const PtLJ<Real>& lj, bool other, const PtCoords<Real>& X, int j, Real xo,
+                                           Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real& en,
+                                           Real& eo, int& cnt)
+{
+  Real xj, yj, zj;
+  X.get(j, xj, yj, zj);
+  const Real bx = xo - xj, by = yo - yj, bz = zo - zj;
+  const Real r2o = PtNum<Real>::keep_or_far(fma(bz, bz, fma(by, by, bx * bx)), other);
+  const Real r2n = fma(tdx, bx, fma(tdy, by, fma(tdz, bz, r2o + dd)));
+  cnt -= lj.add(r2o, eo) ? 1 : 0;
+  cnt += lj.add(r2n, en) ? 1 : 0;
+}
+
+// A5 + the logarithm of A6, one instruction stream for a whole warp: threads with role 0..3 take
+// the bonds (new m-1, new m+1, old m-1, old m+1) of Eq. (3), role 4 takes log(u) for the
+// Metropolis test  u < exp(-beta dE)  <=>  log u < -beta dE  (Eq. 5).  Returns this thread's
+// addend to Delta E; *lg is log(arg) of the role; *broke says a new bond left (r0-R, r0+R).
+template <typename Real>
+__device__ __forceinline__ Real bonds_and_logu(const PtDev& d, int role, int m, int N, const PtCoords<Real>& X,
+                                               Real xo, Real yo, Real zo, Real xn, Real yn, Real zn, Real u,
+                                               Real* lg, bool* broke)
+{
+  const int nb = (role & 1) ? m + 1 : m - 1;
+  const bool isbond = role < 4 && nb >= 0 && nb < N;
+  const bool isnew = role < 2;
+  const int nbc = isbond ? nb : m;
+  Real xb, yb, zb;
+  X.get(nbc, xb, yb, zb);
+  const Real dx = (isnew ? xn : xo) - xb;
+  const Real dy = (isnew ? yn : yo) - yb;
+  const Real dz = (isnew ? zn : zo) - zb;
+  const Real r2 = isbond ? fma(dz, dz, fma(dy, dy, dx * dx)) : (Real)(d.r0 * d.r0);
+  const Real r = PtNum<Real>::sqrt_(r2);
+  const Real q = (r - (Real)d.r0) * (Real)d.invR;
+  const Real g = fma(-q, q, (Real)1);              // 1 - ((r - r0)/R)^2
+  const bool in_range = g > (Real)0;               // false for NaN as well
+  *broke = isbond && isnew && !in_range;
+  const Real arg = role == 4 ? u : ((isbond && in_range) ? g : (Real)1);
+  *lg = PtNum<Real>::log_(arg);
+  const Real fc = isnew ? (Real)d.feneC : (Real)-d.feneC;   // -(K/2) R^2
+  return role < 4 ? fc * *lg : (Real)0;
+}
+
+// Eq. (8), and R_ee once per sweep; all lanes of the group take part.
+template <typename Real, int L>
+__device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const PtCoords<Real>& X)
+{
+  double sx = 0.0, sy = 0.0, sz = 0.0;
+  for (int j = lig; j < N; j += L) {
+    Real x, y, z;
+    X.get(j, x, y, z);
+    sx += (double)x; sy += (double)y; sz += (double)z;
+  }
+  sx = group_sum<double, L>(sx) / (double)N;
+  sy = group_sum<double, L>(sy) / (double)N;
+  sz = group_sum<double, L>(sz) / (double)N;
+  double q = 0.0;
+  for (int j = lig; j < N; j += L) {
+    Real x, y, z;
+    X.get(j, x, y, z);
+    const double dx = (double)x - sx, dy = (double)y - sy, dz = (double)z - sz;
+    q += dx * dx + dy * dy + dz * dz;
+  }
+  const double rg2 = group_sum<double, L>(q) / (double)N;
+  Real x0, y0, z0, x1, y1, z1;
+  X.get(0, x0, y0, z0);
+  X.get(N - 1, x1, y1, z1);
+  const double ex = (double)x1 - (double)x0, ey = (double)y1 - (double)y0, ez = (double)z1 - (double)z0;
+  const double ree2 = ex * ex + ey * ey + ez * ez;
+  c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
+}
+
 // ------------------------------------------------------------------------------------------
-// Warp-group kernel: L lanes per chain, 32/L chains per warp.
+// Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
 // ------------------------------------------------------------------------------------------
 template <typename Real, int L>
 __global__ void __launch_bounds__(128) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
+  static_assert(L >= 8 && L <= 32, "lanes per chain");
   constexpr int G = 32 / L;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int g = lane / L, lig = lane % L;
   const int cl = warp * G + g;
   const int N = d.N, Ns = pl.Ns;
-  const Real FAR = (Real)PT_FAR;
 
   ChainCtx c;
   ctx_load(d, blockIdx.x * pl.chains_per_cta + cl, c);
   const Real width = (Real)d.width[c.i];
   const PtLJ<Real> lj(d);
 
-  Real* xs = reinterpret_cast<Real*>(smem_raw) + (size_t)cl * pl.sstride;
-  Real* ys = xs + Ns;
-  Real* zs = ys + Ns;
+  const PtCoords<Real> X(reinterpret_cast<Real*>(smem_raw) + (size_t)cl * pl.sstride, Ns);
 
-  // A1: HBM -> shared memory, padding entries far away
+  // A1: HBM -> shared memory; padding entries lie far outside every cutoff
   Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
   for (int j = lig; j < Ns; j += L) {
     const bool in = j < N;
-    xs[j] = in ? gx[j] : FAR;
-    ys[j] = in ? gx[d.Ng + j] : FAR;
-    zs[j] = in ? gx[2 * d.Ng + j] : FAR;
+    X.set(j, in ? gx[j] : (Real)PT_FAR, in ? gx[d.Ng + j] : (Real)PT_FAR, in ? gx[2 * d.Ng + j] : (Real)PT_FAR);
   }
   __syncwarp();
 
   const bool pick = d.select_mode == PT_RANDOM_PICK;
   const bool leader = (lig == 0) && c.active;
-  const unsigned bond_lanes = 3u << (g * L);   // lanes 0,1 of the group: the new bonds
+  const unsigned bond_lanes = 3u << (g * L);   // roles 0, 1 of this group: the new bonds
+  const double nbeta = -c.beta;
 
+  Proposal<Real> nx = draw_proposal<Real>(c, pick, N, 0u, t0);
   for (int sw = 0; sw < n_sweeps; ++sw) {
     const uint32_t t = t0 + (uint32_t)sw;
     for (int k = 0; k < N; ++k) {
-      // A2: proposal
-      int m = k;
-      if (pick) {
-        const uint4 wp = pt_draw(c.key, (uint32_t)k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
-        m = (int)__umulhi(wp.x, (uint32_t)N);
+      // A2: this step's proposal was drawn one step ahead; draw the next one now so that the
+      // integer work overlaps the fp64 work below
+      const Proposal<Real> p = nx;
+      {
+        const bool last = k + 1 == N;
+        nx = draw_proposal<Real>(c, pick, N, last ? 0u : (uint32_t)(k + 1), last ? t + 1u : t);
       }
-      const uint4 w = pt_draw(c.key, (uint32_t)k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
-      const Real xo = xs[m], yo = ys[m], zo = zs[m];
-      const Real xn = PtNum<Real>::propose(xo, width, PtNum<Real>::sym(w.x));
-      const Real yn = PtNum<Real>::propose(yo, width, PtNum<Real>::sym(w.y));
-      const Real zn = PtNum<Real>::propose(zo, width, PtNum<Real>::sym(w.z));
-      const Real u = PtNum<Real>::u01(w.w);
-      __syncwarp();
-      // hide monomer m from its own sum: its slot looks like a padding entry during the loop
-      if (lig == 0) { xs[m] = FAR; ys[m] = FAR; zs[m] = FAR; }
-      __syncwarp();
+      const int m = p.m;
+      Real xo, yo, zo;
+      X.get(m, xo, yo, zo);
+      const Real xn = PtNum<Real>::propose(xo, width, p.sx);
+      const Real yn = PtNum<Real>::propose(yo, width, p.sy);
+      const Real zn = PtNum<Real>::propose(zo, width, p.sz);
+      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
+      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
+      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
 
       // A3: Delta E_LJ, lanes stride over partners (Eq. 1, 2)
       Real en = (Real)0, eo = (Real)0;
+      int cnt = 0;
 #pragma unroll 2
-      for (int j = lig; j < Ns; j += L) {
-        const Real xj = xs[j], yj = ys[j], zj = zs[j];
-        const Real ax = xn - xj, ay = yn - yj, az = zn - zj;
-        const Real bx = xo - xj, by = yo - yj, bz = zo - zj;
-        const Real r2n = fma(az, az, fma(ay, ay, ax * ax));
-        const Real r2o = fma(bz, bz, fma(by, by, bx * bx));
-        const Real tn = lj.inside(r2n);
-        const Real to = lj.inside(r2o);
-        if (r2n < lj.rc2) en += tn;
-        if (r2o < lj.rc2) eo += to;
-      }
-      Real part = en - eo;
+      for (int j = lig; j < Ns; j += L)
+        pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
+      Real part = fma(-lj.C, (Real)cnt, en - eo);
 
-      // A5: the <= 2 bonds of m, new and old, one bond per lane (Eq. 3)
-      bool broke = false;
-      if (lig < 4) {
-        const int nb = (lig & 1) ? m + 1 : m - 1;
-        if (nb >= 0 && nb < N) {
-          const bool isnew = lig < 2;
-          const Real dx = (isnew ? xn : xo) - xs[nb];
-          const Real dy = (isnew ? yn : yo) - ys[nb];
-          const Real dz = (isnew ? zn : zo) - zs[nb];
-          bool inside;
-          const Real f = Fene<Real>::eval(d, fma(dz, dz, fma(dy, dy, dx * dx)), &inside);
-          if (isnew) { part += f; broke = !inside; }
-          else part -= f;
-        }
-      }
+      // A5: bonds, and log u of A6
+      Real lg;
+      bool broke;
+      part += bonds_and_logu<Real>(d, lig, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
       const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
+      const Real logu = __shfl_sync(0xffffffffu, lg, g * L + 4);
 
       // A4: reduce; every lane of the group gets the same Delta E
       const Real dE = group_sum<Real, L>(part);
 
-      // A6: Metropolis, Eq. (5)
-      bool accept;
-      if (bond_broken) accept = false;
-      else if (dE <= (Real)0) accept = true;
-      else accept = Fene<Real>::metropolis(u, c.beta, dE);   // NaN compares false: reject
+      // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
+      const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
 
-      // A7: commit (or restore)
+      // A7: commit
       if (lig == 0) {
-        xs[m] = accept ? xn : xo;
-        ys[m] = accept ? yn : yo;
-        zs[m] = accept ? zn : zo;
+        if (accept) X.set(m, xn, yn, zn);
         if (d.tr_move && c.active && (long long)t < d.cap_sweeps)
           d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
       }
@@ -232,31 +278,14 @@ __global__ void __launch_bounds__(128) k_sweep_group(const PtDev d, const PtLaun
     }
 
     // A8: measurement once per sweep
-    if (d.observables) {
-      // Eq. (8): r_gyr^2 = (1/N) sum_k (r_k - r_mean)^2; R_ee^2 = |r_N - r_1|^2
-      double sx = 0.0, sy = 0.0, sz = 0.0;
-      for (int j = lig; j < N; j += L) { sx += (double)xs[j]; sy += (double)ys[j]; sz += (double)zs[j]; }
-      sx = group_sum<double, L>(sx) / (double)N;
-      sy = group_sum<double, L>(sy) / (double)N;
-      sz = group_sum<double, L>(sz) / (double)N;
-      double q = 0.0;
-      for (int j = lig; j < N; j += L) {
-        const double dx = (double)xs[j] - sx, dy = (double)ys[j] - sy, dz = (double)zs[j] - sz;
-        q += dx * dx + dy * dy + dz * dz;
-      }
-      const double rg2 = group_sum<double, L>(q) / (double)N;
-      const double ex = (double)xs[N - 1] - (double)xs[0], ey = (double)ys[N - 1] - (double)ys[0],
-                   ez = (double)zs[N - 1] - (double)zs[0];
-      const double ree2 = ex * ex + ey * ey + ez * ez;
-      c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
-    }
+    if (d.observables) measure_shape<Real, L>(c, N, lig, X);
     if (leader) measure_energy(d, c, t);
   }
 
   // A9: shared memory -> HBM
   __syncwarp();
   if (c.active) {
-    for (int j = lig; j < N; j += L) { gx[j] = xs[j]; gx[d.Ng + j] = ys[j]; gx[2 * d.Ng + j] = zs[j]; }
+    for (int j = lig; j < N; j += L) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
     if (lig == 0) ctx_store(d, c, n_sweeps);
   }
 }
@@ -270,72 +299,58 @@ __global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ double red[2][8];
+  __shared__ double s_logu[2];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int T = blockDim.x, NW = T >> 5;
   const int N = d.N, Ns = pl.Ns;
-  const Real FAR = (Real)PT_FAR;
 
   ChainCtx c;
   ctx_load(d, blockIdx.x, c);
   const Real width = (Real)d.width[c.i];
   const PtLJ<Real> lj(d);
 
-  Real* xs = reinterpret_cast<Real*>(smem_raw);
-  Real* ys = xs + Ns;
-  Real* zs = ys + Ns;
+  const PtCoords<Real> X(reinterpret_cast<Real*>(smem_raw), Ns);
   Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
   for (int j = tid; j < Ns; j += T) {
     const bool in = j < N;
-    xs[j] = in ? gx[j] : FAR;
-    ys[j] = in ? gx[d.Ng + j] : FAR;
-    zs[j] = in ? gx[2 * d.Ng + j] : FAR;
+    X.set(j, in ? gx[j] : (Real)PT_FAR, in ? gx[d.Ng + j] : (Real)PT_FAR, in ? gx[2 * d.Ng + j] : (Real)PT_FAR);
   }
   __syncthreads();
 
   const bool pick = d.select_mode == PT_RANDOM_PICK;
+  const double nbeta = -c.beta;
+  Proposal<Real> nx = draw_proposal<Real>(c, pick, N, 0u, t0);
   for (int sw = 0; sw < n_sweeps; ++sw) {
     const uint32_t t = t0 + (uint32_t)sw;
     for (int k = 0; k < N; ++k) {
-      int m = k;
-      if (pick) {
-        const uint4 wp = pt_draw(c.key, (uint32_t)k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
-        m = (int)__umulhi(wp.x, (uint32_t)N);
+      const Proposal<Real> p = nx;
+      {
+        const bool last = k + 1 == N;
+        nx = draw_proposal<Real>(c, pick, N, last ? 0u : (uint32_t)(k + 1), last ? t + 1u : t);
       }
-      const uint4 w = pt_draw(c.key, (uint32_t)k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
-      const Real xo = xs[m], yo = ys[m], zo = zs[m];
-      const Real xn = PtNum<Real>::propose(xo, width, PtNum<Real>::sym(w.x));
-      const Real yn = PtNum<Real>::propose(yo, width, PtNum<Real>::sym(w.y));
-      const Real zn = PtNum<Real>::propose(zo, width, PtNum<Real>::sym(w.z));
-      const Real u = PtNum<Real>::u01(w.w);
+      const int m = p.m;
+      Real xo, yo, zo;
+      X.get(m, xo, yo, zo);
+      const Real xn = PtNum<Real>::propose(xo, width, p.sx);
+      const Real yn = PtNum<Real>::propose(yo, width, p.sy);
+      const Real zn = PtNum<Real>::propose(zo, width, p.sz);
+      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
+      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
+      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
 
       Real en = (Real)0, eo = (Real)0;
+      int cnt = 0;
 #pragma unroll 2
-      for (int j = tid; j < Ns; j += T) {
-        const Real xj = xs[j], yj = ys[j], zj = zs[j];
-        const Real ax = xn - xj, ay = yn - yj, az = zn - zj;
-        const Real bx = xo - xj, by = yo - yj, bz = zo - zj;
-        const Real r2n = fma(az, az, fma(ay, ay, ax * ax));
-        const Real r2o = fma(bz, bz, fma(by, by, bx * bx));
-        const Real tn = lj.inside(r2n);
-        const Real to = lj.inside(r2o);
-        const bool other = j != m;
-        if (other && r2n < lj.rc2) en += tn;
-        if (other && r2o < lj.rc2) eo += to;
-      }
-      Real part = en - eo;
+      for (int j = tid; j < Ns; j += T)
+        pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
+      Real part = fma(-lj.C, (Real)cnt, en - eo);
+
+      // bonds and log u: roles 0..4 are threads 0..4 of warp 0; the other warps skip the stream
       bool broke = false;
-      if (tid < 4) {
-        const int nb = (tid & 1) ? m + 1 : m - 1;
-        if (nb >= 0 && nb < N) {
-          const bool isnew = tid < 2;
-          const Real dx = (isnew ? xn : xo) - xs[nb];
-          const Real dy = (isnew ? yn : yo) - ys[nb];
-          const Real dz = (isnew ? zn : zo) - zs[nb];
-          bool inside;
-          const Real f = Fene<Real>::eval(d, fma(dz, dz, fma(dy, dy, dx * dx)), &inside);
-          if (isnew) { part += f; broke = !inside; }
-          else part -= f;
-        }
+      if (warp == 0) {
+        Real lg;
+        part += bonds_and_logu<Real>(d, lane, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
+        if (lane == 4) s_logu[k & 1] = (double)lg;
       }
       const Real wsum = group_sum<Real, 32>(part);
       if (lane == 0) red[k & 1][warp] = (double)wsum;
@@ -343,14 +358,12 @@ __global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch
       double dEd = red[k & 1][0];
       for (int q = 1; q < NW; ++q) dEd += red[k & 1][q];
       const Real dE = (Real)dEd;
+      const double logu = s_logu[k & 1];
 
-      bool accept;
-      if (bond_broken) accept = false;
-      else if (dE <= (Real)0) accept = true;
-      else accept = Fene<Real>::metropolis(u, c.beta, dE);
+      const bool accept = !bond_broken && (dE <= (Real)0 || logu < nbeta * (double)dE);
 
       if (tid == 0) {
-        if (accept) { xs[m] = xn; ys[m] = yn; zs[m] = zn; }
+        if (accept) X.set(m, xn, yn, zn);
         if (d.tr_move && (long long)t < d.cap_sweeps)
           d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
       }
@@ -359,28 +372,12 @@ __global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch
       __syncthreads();
     }
 
-    if (d.observables && warp == 0) {
-      double sx = 0.0, sy = 0.0, sz = 0.0;
-      for (int j = lane; j < N; j += 32) { sx += (double)xs[j]; sy += (double)ys[j]; sz += (double)zs[j]; }
-      sx = group_sum<double, 32>(sx) / (double)N;
-      sy = group_sum<double, 32>(sy) / (double)N;
-      sz = group_sum<double, 32>(sz) / (double)N;
-      double q = 0.0;
-      for (int j = lane; j < N; j += 32) {
-        const double dx = (double)xs[j] - sx, dy = (double)ys[j] - sy, dz = (double)zs[j] - sz;
-        q += dx * dx + dy * dy + dz * dz;
-      }
-      const double rg2 = group_sum<double, 32>(q) / (double)N;
-      const double ex = (double)xs[N - 1] - (double)xs[0], ey = (double)ys[N - 1] - (double)ys[0],
-                   ez = (double)zs[N - 1] - (double)zs[0];
-      const double ree2 = ex * ex + ey * ey + ez * ez;
-      c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
-    }
+    if (d.observables && warp == 0) measure_shape<Real, 32>(c, N, lane, X);
     if (tid == 0) measure_energy(d, c, t);
   }
 
   __syncthreads();
-  for (int j = tid; j < N; j += T) { gx[j] = xs[j]; gx[d.Ng + j] = ys[j]; gx[2 * d.Ng + j] = zs[j]; }
+  for (int j = tid; j < N; j += T) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
   if (tid == 0) ctx_store(d, c, n_sweeps);
 }
 
@@ -391,7 +388,6 @@ template <typename Real> cudaError_t launch_t(const PtDev& d, const PtLaunch& pl
 {
   const dim3 grid(pl.grid), block(pl.threads);
   switch (pl.lanes) {
-    case 4: k_sweep_group<Real, 4><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
     case 8: k_sweep_group<Real, 8><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
     case 16: k_sweep_group<Real, 16><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
     case 32: k_sweep_group<Real, 32><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
@@ -414,7 +410,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     else {
       L = 32;
       while (L > 8 && (long long)d.C * (L / 2) / 32 >= 2 * smsp && d.N > L / 2) L /= 2;
-      while (L > 4 && L / 2 >= d.N) L /= 2;
+      while (L > 8 && L / 2 >= d.N) L /= 2;
     }
   }
   PtLaunch pl{};
@@ -453,12 +449,10 @@ cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, u
   static bool attr_done = false;
   if (!attr_done) {
     const int big = 200 * 1024;
-    cudaFuncSetAttribute(k_sweep_group<double, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<double, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<double, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<double, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_cta<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<float, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<float, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<float, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
     cudaFuncSetAttribute(k_sweep_group<float, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
