@@ -85,8 +85,45 @@ template <> struct PtNum<double> {
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
   }
-  static __device__ __forceinline__ double sqrt_(double v) { return sqrt(v); }
-  static __device__ __forceinline__ double log_(double v) { return log(v); }
+  // sqrt(a) for a normal a > 0, branch-free so that it can be scheduled between the pair terms:
+  // y = MUFU.RSQ64H seed (relative error eps < 2^-19), g = a y, r = (1 - a y^2)/2, and
+  // sqrt(a) = g (1 - 2r)^(-1/2) = g (1 + r + 3/2 r^2 + O(r^3)); truncation < 2^-60.  a = 0 gives
+  // NaN (callers treat NaN as "outside the FENE range").  6 fp64-pipe instructions.
+  static __device__ __forceinline__ double sqrt_(double a)
+  {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double g = a * y, h = 0.5 * y;
+    const double r = fma(-h, g, 0.5);
+    const double t = fma(1.5 * r, r, r);
+    return fma(g, t, g);
+  }
+  // log(v) for a normal v > 0, branch-free.  v = 2^e m with m in [sqrt(1/2), sqrt(2)) by integer
+  // arithmetic on the high word; log m = 2 atanh(s), s = (m - 1)/(m + 1), |s| < 0.1716, as the
+  // odd Taylor series 2 s (1 + z/3 + z^2/5 + ... + z^10/21), z = s^2 (next term < 2^-60 relative);
+  // log v = e ln2_hi + (e ln2_lo + log m).  No cancellation near v = 1 because e = 0 there.
+  static __device__ __forceinline__ double log_(double v)
+  {
+    const int hi = __double2hiint(v);
+    const int e = (hi - 0x3fe6a09e) >> 20;          // floor: high word of sqrt(1/2) is 0x3fe6a09e
+    const double m = __hiloint2double(hi - (e << 20), __double2loint(v));
+    const double f = m - 1.0;
+    const double s = f * rcp(m + 1.0);
+    const double z = s * s;
+    double p = 2.0 / 21.0;
+    p = fma(p, z, 2.0 / 19.0);
+    p = fma(p, z, 2.0 / 17.0);
+    p = fma(p, z, 2.0 / 15.0);
+    p = fma(p, z, 2.0 / 13.0);
+    p = fma(p, z, 2.0 / 11.0);
+    p = fma(p, z, 2.0 / 9.0);
+    p = fma(p, z, 2.0 / 7.0);
+    p = fma(p, z, 2.0 / 5.0);
+    p = fma(p, z, 2.0 / 3.0);
+    const double logm = fma(s, p * z, s + s);
+    const double de = (double)e;
+    return fma(de, 0x1.62e42fefa39efp-1, fma(de, 0x1.abc9e3b39803fp-56, logm));
+  }
 };
 
 template <> struct PtNum<float> {

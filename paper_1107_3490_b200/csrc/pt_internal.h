@@ -54,6 +54,7 @@ struct PtLaunch {
   int smem_bytes;      // dynamic shared memory per CTA
   int sstride;         // shared-memory stride between chains, in Reals
   int Ns;              // padded monomers per coordinate array in shared memory
+  int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
 };
 
 // pt_sweep.cu

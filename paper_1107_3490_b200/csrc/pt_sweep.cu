@@ -192,8 +192,11 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const
 // ------------------------------------------------------------------------------------------
 // Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
 // ------------------------------------------------------------------------------------------
-template <typename Real, int L>
-__global__ void __launch_bounds__(128) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
+// NI > 0: the partner loop has exactly NI iterations (Ns = NI * L) and is unrolled completely, so
+// that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
+// pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
+template <typename Real, int L, int NI>
+__global__ void __launch_bounds__(256) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -245,18 +248,26 @@ __global__ void __launch_bounds__(128) k_sweep_group(const PtDev d, const PtLaun
       const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
       const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
 
-      // A3: Delta E_LJ, lanes stride over partners (Eq. 1, 2)
-      Real en = (Real)0, eo = (Real)0;
-      int cnt = 0;
-#pragma unroll 2
-      for (int j = lig; j < Ns; j += L)
-        pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
-      Real part = fma(-lj.C, (Real)cnt, en - eo);
-
       // A5: bonds, and log u of A6
       Real lg;
       bool broke;
-      part += bonds_and_logu<Real>(d, lig, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
+      const Real bond = bonds_and_logu<Real>(d, lig, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
+
+      // A3: Delta E_LJ, lanes stride over partners (Eq. 1, 2)
+      Real en = (Real)0, eo = (Real)0;
+      int cnt = 0;
+      if (NI > 0) {
+#pragma unroll
+        for (int it = 0; it < NI; ++it) {
+          const int j = lig + it * L;
+          pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
+        }
+      } else {
+#pragma unroll 2
+        for (int j = lig; j < Ns; j += L)
+          pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
+      }
+      const Real part = fma(-lj.C, (Real)cnt, en - eo) + bond;
       const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
       const Real logu = __shfl_sync(0xffffffffu, lg, g * L + 4);
 
@@ -383,17 +394,36 @@ __global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch
 
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
-template <typename Real> cudaError_t launch_t(const PtDev& d, const PtLaunch& pl, uint32_t t0, int n,
-                                              cudaStream_t st)
+typedef void (*SweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
+
+struct SweepVariant {
+  int L, NI;
+  SweepFn f64, f32;
+};
+
+#define PT_VARIANT(L, NI) { L, NI, k_sweep_group<double, L, NI>, k_sweep_group<float, L, NI> }
+// Unrolled instantiations (NI = partner-loop iterations); NI = 0 is the run-time loop of the same
+// lane count and must come last within its L.
+const SweepVariant kVariants[] = {
+    PT_VARIANT(8, 2),  PT_VARIANT(8, 4),  PT_VARIANT(8, 7),  PT_VARIANT(8, 10), PT_VARIANT(8, 13),
+    PT_VARIANT(8, 0),
+    PT_VARIANT(16, 1), PT_VARIANT(16, 2), PT_VARIANT(16, 4), PT_VARIANT(16, 7), PT_VARIANT(16, 0),
+    PT_VARIANT(32, 1), PT_VARIANT(32, 2), PT_VARIANT(32, 4), PT_VARIANT(32, 0),
+};
+
+const SweepVariant* find_variant(int L, int ni_needed)
 {
-  const dim3 grid(pl.grid), block(pl.threads);
-  switch (pl.lanes) {
-    case 8: k_sweep_group<Real, 8><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
-    case 16: k_sweep_group<Real, 16><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
-    case 32: k_sweep_group<Real, 32><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
-    default: k_sweep_cta<Real><<<grid, block, pl.smem_bytes, st>>>(d, pl, t0, n); break;
-  }
-  return cudaGetLastError();
+  for (const SweepVariant& v : kVariants)
+    if (v.L == L && (v.NI == 0 || v.NI >= ni_needed)) return &v;
+  return nullptr;
+}
+
+SweepFn kernel_of(const PtLaunch& pl, int precision)
+{
+  if (pl.lanes > 32) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
+  for (const SweepVariant& v : kVariants)
+    if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32 : v.f64;
+  return nullptr;
 }
 
 }  // namespace
@@ -401,15 +431,25 @@ template <typename Real> cudaError_t launch_t(const PtDev& d, const PtLaunch& pl
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan)
 {
   const int real_bytes = precision == PT_F32 ? 4 : 8;
+  int sms = 148;
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) {
+      int v = 0;
+      if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
+    }
+    cudaGetLastError();
+  }
+  const long long smsp = 4ll * sms;
   int L = lanes_requested;
   if (L == 0) {
-    // Few long chains: one CTA per replica.  Otherwise as few lanes per chain as still give every
-    // SM sub-partition a warp (the serial part of a step is shared by the 32/L chains of a warp).
-    const long long smsp = 148ll * 4;
-    if (d.N >= 192 && (long long)d.C * 4 <= 2 * smsp) L = 128;
+    // Few long chains: one CTA per replica.  Otherwise the fewest lanes per chain that still give
+    // every SM sub-partition a warp: the serial part of a step (proposal, bonds, log u, decision)
+    // is one instruction stream shared by the 32/L chains of a warp.
+    if (d.N >= 192 && (long long)d.C <= smsp) L = 128;
     else {
       L = 32;
-      while (L > 8 && (long long)d.C * (L / 2) / 32 >= 2 * smsp && d.N > L / 2) L /= 2;
+      while (L > 8 && ((long long)d.C * (L / 2) + 31) / 32 >= smsp && d.N > L / 2) L /= 2;
       while (L > 8 && L / 2 >= d.N) L /= 2;
     }
   }
@@ -417,20 +457,30 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   pl.lanes = L;
   if (L <= 32) {
     const int G = 32 / L;
-    pl.Ns = round_up(d.N, L);
+    const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
+    if (!v) return cudaErrorInvalidValue;
+    pl.ni = v->NI;
+    pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
     // chains of one warp must start in different banks: stride = L (mod Q) words, where Q words
     // span all 32 banks (fp64: a warp's 8-byte loads go in two phases of 16 lanes, Q = 16)
     const int Q = 128 / real_bytes;
     int ss = 3 * pl.Ns;
     while (ss % Q != L % Q) ++ss;
     pl.sstride = ss;
+    // one CTA per SM when there are enough warps (its warps are dealt round-robin to the four
+    // sub-partitions, so they are balanced by construction); single-warp CTAs otherwise
     const long long warps = ((long long)d.C + G - 1) / G;
-    const int wpc = warps <= 148ll * 24 ? 1 : 4;
+    int wpc = 1;
+    if (warps > sms) {
+      wpc = (int)((warps + sms - 1) / sms);
+      if (wpc > 8) wpc = 8;
+    }
     pl.threads = 32 * wpc;
     pl.chains_per_cta = G * wpc;
     pl.grid = (int)((d.C + pl.chains_per_cta - 1) / pl.chains_per_cta);
     pl.smem_bytes = pl.chains_per_cta * pl.sstride * real_bytes;
   } else {
+    pl.ni = 0;
     pl.Ns = round_up(d.N, L);
     pl.sstride = 3 * pl.Ns;
     pl.threads = L;
@@ -439,6 +489,12 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.smem_bytes = pl.sstride * real_bytes;
   }
   if (pl.smem_bytes > 200 * 1024) return cudaErrorInvalidValue;
+  SweepFn fn = kernel_of(pl, precision);
+  if (!fn) return cudaErrorInvalidValue;
+  if (pl.smem_bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem_bytes);
+    if (e != cudaSuccess) return e;
+  }
   *plan = pl;
   return cudaSuccess;
 }
@@ -446,21 +502,8 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
 cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, uint32_t t0, int n_sweeps,
                             cudaStream_t stream)
 {
-  static bool attr_done = false;
-  if (!attr_done) {
-    const int big = 200 * 1024;
-    cudaFuncSetAttribute(k_sweep_group<double, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<double, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<double, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_cta<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<float, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<float, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_group<float, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaFuncSetAttribute(k_sweep_cta<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, big);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
-  return precision == PT_F32 ? launch_t<float>(d, pl, t0, n_sweeps, stream)
-                             : launch_t<double>(d, pl, t0, n_sweeps, stream);
+  SweepFn fn = kernel_of(pl, precision);
+  if (!fn) return cudaErrorInvalidValue;
+  fn<<<dim3(pl.grid), dim3(pl.threads), pl.smem_bytes, stream>>>(d, pl, t0, n_sweeps);
+  return cudaGetLastError();
 }
