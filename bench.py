@@ -36,7 +36,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12     # 37.2: 148 SMs x 64 fp
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 * 1e-12    # 74.4
 # fp64-pipe warp instructions the sweep kernel issues per attempted move at the default mapping of
 # config 5, counted in the SASS of the shipped kernel; used for pipe_frac.
-SWEEP_DRAM_TRAFFIC = None         # bytes per sweep launch from ncu --set full (profiles/), None = not captured
+SWEEP_DRAM_TRAFFIC = 12.8e6       # dram read+write bytes per sweep launch of config 5 fp64, ncu --set full (profiles/r01_*_ncu_full.md)
 
 
 def parse_args():
@@ -290,7 +290,7 @@ def run_ours(args, rank, world, local):
     achieved = flops_per_launch / k_s * 1e-12
     peak = pt.pt_fma_peak(pt.PT_F32 if f32 else pt.PT_F64, stream=stream)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": SWEEP_DRAM_TRAFFIC, "kernel": "k_sweep", "kernel_ms": k_s * 1e3,
+                "traffic": SWEEP_DRAM_TRAFFIC if (args.config == 5 and not f32) else None, "kernel": "k_sweep", "kernel_ms": k_s * 1e3,
                 "peak_kind": f"measured {'fp32' if f32 else 'fp64'} FMA chain (pt_fma_peak), this run",
                 "peak_nominal": NOMINAL_FP32_TFLOPS if f32 else NOMINAL_FP64_TFLOPS,
                 "flops_per_pair_eval": FLOPS_PER_PAIR_EVAL,
