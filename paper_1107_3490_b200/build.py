@@ -17,10 +17,10 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpt_b200.so"
-SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu"]
+SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_sweep_spec_f64.cu", "pt_sweep_spec_f32.cu", "pt_peak.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-O3", "-std=c++17", "-lineinfo",
+    "-O3", "-std=c++17", "-lineinfo", "--threads", "0",
     "-shared", "-Xcompiler", "-fPIC",
     "-I", str(ROOT / "include"), "-I", str(CSRC),
 ]
@@ -35,7 +35,7 @@ def _nvcc() -> str:
 
 def _inputs():
     files = [CSRC / s for s in SOURCES]
-    files += sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.cuh"))
+    files += sorted(CSRC.glob("*.h")) + sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.inl"))
     files.append(ROOT / "include" / "pt_b200.h")
     return files
 

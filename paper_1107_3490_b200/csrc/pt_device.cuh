@@ -63,6 +63,14 @@ template <> struct PtNum<double> {
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
   }
+  // the seed of rcp() alone, and whether it needs the Newton step
+  static constexpr bool kNewton = true;
+  static __device__ __forceinline__ double rcp_seed(double d)
+  {
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    return x;
+  }
   // r2 < rc2 for r2 >= 0 (or NaN), decided on the integer pipe: the bit patterns of non-negative
   // doubles are ordered like the numbers; NaN and anything with the sign bit set compare false.
   static __device__ __forceinline__ bool below(double r2, double rc2)
@@ -84,6 +92,15 @@ template <> struct PtNum<double> {
     x = __hiloint2double(inside ? __double2hiint(x) : 0, __double2loint(x));
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
+  }
+  // Eq. (1) literally: E_LJ(min(r, r_c)).  Returns r2 if it lies below rc2 and `keep` holds, else
+  // rc2; compare and select on the integer pipe (bit patterns of non-negative doubles are ordered
+  // like the numbers; NaN and negative values compare false and clamp).
+  static __device__ __forceinline__ double clamp_below(double r2, double rc2, bool keep)
+  {
+    const bool in = below(r2, rc2) && keep;
+    return __hiloint2double(in ? __double2hiint(r2) : __double2hiint(rc2),
+                            in ? __double2loint(r2) : __double2loint(rc2));
   }
   // sqrt(a) for a normal a > 0, branch-free so that it can be scheduled between the pair terms:
   // y = MUFU.RSQ64H seed (relative error eps < 2^-19), g = a y, r = (1 - a y^2)/2, and
@@ -145,6 +162,8 @@ template <> struct PtNum<float> {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return x;
   }
+  static constexpr bool kNewton = false;
+  static __device__ __forceinline__ float rcp_seed(float d) { return rcp(d); }
   static __device__ __forceinline__ bool below(float r2, float rc2) { return r2 < rc2; }
   static __device__ __forceinline__ float keep_or_far(float v, bool keep)
   {
@@ -155,6 +174,10 @@ template <> struct PtNum<float> {
     float x;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return inside ? x : 0.0f;
+  }
+  static __device__ __forceinline__ float clamp_below(float r2, float rc2, bool keep)
+  {
+    return (r2 < rc2 && keep) ? r2 : rc2;
   }
   static __device__ __forceinline__ float sqrt_(float v) { return sqrtf(v); }
   // the paper's fp32 kernels use the fast-math intrinsics (__logf)
@@ -180,6 +203,15 @@ template <typename Real> struct PtLJ {
     const Real u = inv * inv * inv;
     acc = fma(u, fma(A, u, nB), acc);
     return inside;
+  }
+  // acc += u (A u - B) at min(r2, rc2), or at rc2 if !keep: every call adds a term, the ones outside
+  // the cutoff (and the masked ones) add the constant E_LJ(r_c), which cancels between the sum over
+  // new and the sum over old distances because both have the same number of terms.
+  __device__ __forceinline__ void addc(Real r2, bool keep, Real& acc) const
+  {
+    const Real inv = PtNum<Real>::rcp(PtNum<Real>::clamp_below(r2, rc2, keep));
+    const Real u = inv * inv * inv;
+    acc = fma(u, fma(A, u, nB), acc);
   }
 };
 

@@ -10,184 +10,12 @@
 // recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
 // long chains, and with the local Delta-E of Eq. (5) instead of the full sum.
 #include <math.h>
+#include <stdlib.h>
+#include <string.h>
 
-#include "pt_device.cuh"
+#include "pt_sweep_common.cuh"
 
 namespace {
-
-template <typename Real, int L> __device__ __forceinline__ Real group_sum(Real v)
-{
-#pragma unroll
-  for (int o = L / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
-
-// Everything a chain carries through a launch besides its coordinates.
-struct ChainCtx {
-  int s, e, i, ti;
-  bool active;
-  double beta;
-  uint2 key;
-  double erun, mom1, mom2;
-  double ob0, ob1, ob2, ob3;
-  unsigned acc, brej;
-};
-
-__device__ __forceinline__ void ctx_load(const PtDev& d, int s, ChainCtx& c)
-{
-  c.active = s < d.C;
-  c.s = c.active ? s : d.C - 1;
-  c.e = c.s / d.M;
-  c.i = d.temp_of_slot[c.s];
-  c.ti = c.e * d.M + c.i;
-  c.beta = d.beta[c.i];
-  c.key = d.keys[c.e];
-  c.erun = d.erun[c.s];
-  c.mom1 = d.mom[3 * c.ti + 1];
-  c.mom2 = d.mom[3 * c.ti + 2];
-  c.ob0 = d.obs[4 * c.ti + 0];
-  c.ob1 = d.obs[4 * c.ti + 1];
-  c.ob2 = d.obs[4 * c.ti + 2];
-  c.ob3 = d.obs[4 * c.ti + 3];
-  c.acc = 0;
-  c.brej = 0;
-}
-
-// once per sweep, by one thread of the chain (A8): histogram, moments, energy trace
-__device__ __forceinline__ void measure_energy(const PtDev& d, ChainCtx& c, uint32_t t)
-{
-  const double E = c.erun;
-  if (d.nbins > 0) {
-    const double b = floor((E - d.hist_emin) * d.hist_scale);
-    int idx;
-    if (b >= 0.0 && b < (double)d.nbins) idx = (int)b;
-    else if (b < 0.0) idx = d.nbins;       // underflow
-    else idx = d.nbins + 1;                // overflow (and NaN)
-    // temperature index ti is owned by exactly one chain during a launch: no atomic needed
-    d.hist[(size_t)c.ti * (size_t)(d.nbins + 2) + idx] += 1ull;
-  }
-  c.mom1 = __dadd_rn(c.mom1, E);
-  c.mom2 = __dadd_rn(c.mom2, __dmul_rn(E, E));
-  if (d.tr_e && (long long)t < d.cap_sweeps) d.tr_e[(size_t)c.ti * d.cap_sweeps + t] = E;
-}
-
-__device__ __forceinline__ void ctx_store(const PtDev& d, const ChainCtx& c, int n_sweeps)
-{
-  d.erun[c.s] = c.erun;
-  d.mom[3 * c.ti + 0] += (double)n_sweeps;
-  d.mom[3 * c.ti + 1] = c.mom1;
-  d.mom[3 * c.ti + 2] = c.mom2;
-  if (d.observables) {
-    d.obs[4 * c.ti + 0] = c.ob0;
-    d.obs[4 * c.ti + 1] = c.ob1;
-    d.obs[4 * c.ti + 2] = c.ob2;
-    d.obs[4 * c.ti + 3] = c.ob3;
-  }
-  d.mcount[3 * c.ti + 0] += (unsigned long long)n_sweeps * (unsigned long long)d.N;
-  d.mcount[3 * c.ti + 1] += c.acc;
-  d.mcount[3 * c.ti + 2] += c.brej;
-}
-
-// The proposal of one step (A2): which monomer, where to, and the acceptance uniform.
-template <typename Real> struct Proposal {
-  int m;
-  Real sx, sy, sz, u;
-};
-
-template <typename Real>
-__device__ __forceinline__ Proposal<Real> draw_proposal(const ChainCtx& c, bool pick, int N, uint32_t k, uint32_t t)
-{
-  Proposal<Real> p;
-  p.m = (int)k;
-  if (pick) {   // "a random monomer of the chain is picked"
-    const uint4 wp = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
-    p.m = (int)__umulhi(wp.x, (uint32_t)N);
-  }
-  const uint4 w = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
-  p.sx = PtNum<Real>::sym(w.x);
-  p.sy = PtNum<Real>::sym(w.y);
-  p.sz = PtNum<Real>::sym(w.z);
-  p.u = PtNum<Real>::u01(w.w);
-  return p;
-}
-
-// A3 for one partner j (other = "j is not the moved monomer"): adds u (A u - B) of the new and of
-// the old distance to en / eo when inside the cutoff and counts the inside pairs (cnt = #new - #old)
-// for the shift -C.  The new squared distance follows from the old one:
-// |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2 with b = x_m - x_j.  Branch-free: the moved monomer
-// itself is pushed to a huge distance, pairs outside the cutoff contribute u = 0.
-template <typename Real>
-__device__ __forceinline__ void pair_terms(const PtLJ<Real>& lj, bool other, const PtCoords<Real>& X, int j, Real xo,
-                                           Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real& en,
-                                           Real& eo, int& cnt)
-{
-  Real xj, yj, zj;
-  X.get(j, xj, yj, zj);
-  const Real bx = xo - xj, by = yo - yj, bz = zo - zj;
-  const Real r2o = PtNum<Real>::keep_or_far(fma(bz, bz, fma(by, by, bx * bx)), other);
-  const Real r2n = fma(tdx, bx, fma(tdy, by, fma(tdz, bz, r2o + dd)));
-  cnt -= lj.add(r2o, eo) ? 1 : 0;
-  cnt += lj.add(r2n, en) ? 1 : 0;
-}
-
-// A5 + the logarithm of A6, one instruction stream for a whole warp: threads with role 0..3 take
-// the bonds (new m-1, new m+1, old m-1, old m+1) of Eq. (3), role 4 takes log(u) for the
-// Metropolis test  u < exp(-beta dE)  <=>  log u < -beta dE  (Eq. 5).  Returns this thread's
-// addend to Delta E; *lg is log(arg) of the role; *broke says a new bond left (r0-R, r0+R).
-template <typename Real>
-__device__ __forceinline__ Real bonds_and_logu(const PtDev& d, int role, int m, int N, const PtCoords<Real>& X,
-                                               Real xo, Real yo, Real zo, Real xn, Real yn, Real zn, Real u,
-                                               Real* lg, bool* broke)
-{
-  const int nb = (role & 1) ? m + 1 : m - 1;
-  const bool isbond = role < 4 && nb >= 0 && nb < N;
-  const bool isnew = role < 2;
-  const int nbc = isbond ? nb : m;
-  Real xb, yb, zb;
-  X.get(nbc, xb, yb, zb);
-  const Real dx = (isnew ? xn : xo) - xb;
-  const Real dy = (isnew ? yn : yo) - yb;
-  const Real dz = (isnew ? zn : zo) - zb;
-  const Real r2 = isbond ? fma(dz, dz, fma(dy, dy, dx * dx)) : (Real)(d.r0 * d.r0);
-  const Real r = PtNum<Real>::sqrt_(r2);
-  const Real q = (r - (Real)d.r0) * (Real)d.invR;
-  const Real g = fma(-q, q, (Real)1);              // 1 - ((r - r0)/R)^2
-  const bool in_range = g > (Real)0;               // false for NaN as well
-  *broke = isbond && isnew && !in_range;
-  const Real arg = role == 4 ? u : ((isbond && in_range) ? g : (Real)1);
-  *lg = PtNum<Real>::log_(arg);
-  const Real fc = isnew ? (Real)d.feneC : (Real)-d.feneC;   // -(K/2) R^2
-  return role < 4 ? fc * *lg : (Real)0;
-}
-
-// Eq. (8), and R_ee once per sweep; all lanes of the group take part.
-template <typename Real, int L>
-__device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const PtCoords<Real>& X)
-{
-  double sx = 0.0, sy = 0.0, sz = 0.0;
-  for (int j = lig; j < N; j += L) {
-    Real x, y, z;
-    X.get(j, x, y, z);
-    sx += (double)x; sy += (double)y; sz += (double)z;
-  }
-  sx = group_sum<double, L>(sx) / (double)N;
-  sy = group_sum<double, L>(sy) / (double)N;
-  sz = group_sum<double, L>(sz) / (double)N;
-  double q = 0.0;
-  for (int j = lig; j < N; j += L) {
-    Real x, y, z;
-    X.get(j, x, y, z);
-    const double dx = (double)x - sx, dy = (double)y - sy, dz = (double)z - sz;
-    q += dx * dx + dy * dy + dz * dz;
-  }
-  const double rg2 = group_sum<double, L>(q) / (double)N;
-  Real x0, y0, z0, x1, y1, z1;
-  X.get(0, x0, y0, z0);
-  X.get(N - 1, x1, y1, z1);
-  const double ex = (double)x1 - (double)x0, ey = (double)y1 - (double)y0, ez = (double)z1 - (double)z0;
-  const double ree2 = ex * ex + ey * ey + ez * ez;
-  c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
-}
 
 // ------------------------------------------------------------------------------------------
 // Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
@@ -196,7 +24,7 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const
 // that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
 // pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
 template <typename Real, int L, int NI>
-__global__ void __launch_bounds__(256) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
+__global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -305,7 +133,7 @@ __global__ void __launch_bounds__(256) k_sweep_group(const PtDev d, const PtLaun
 // CTA-per-replica kernel: blockDim.x threads share one chain (long chains, few replicas).
 // ------------------------------------------------------------------------------------------
 template <typename Real>
-__global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch pl, const uint32_t t0,
+__global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                    const int n_sweeps)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -394,7 +222,7 @@ __global__ void __launch_bounds__(256) k_sweep_cta(const PtDev d, const PtLaunch
 
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
-typedef void (*SweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
+typedef PtSweepFn SweepFn;
 
 struct SweepVariant {
   int L, NI;
@@ -418,9 +246,11 @@ const SweepVariant* find_variant(int L, int ni_needed)
   return nullptr;
 }
 
-SweepFn kernel_of(const PtLaunch& pl, int precision)
+SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
-  if (pl.lanes > 32) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
+  if (pl.kind == PT_K_CTA) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
+  if (pl.kind == PT_K_SPEC)
+    return precision == PT_F32 ? pt_spec_kernel_f32(pl.lanes, pl.ni, trace) : pt_spec_kernel_f64(pl.lanes, pl.ni, trace);
   for (const SweepVariant& v : kVariants)
     if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32 : v.f64;
   return nullptr;
@@ -457,10 +287,24 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   pl.lanes = L;
   if (L <= 32) {
     const int G = 32 / L;
-    const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
-    if (!v) return cudaErrorInvalidValue;
-    pl.ni = v->NI;
-    pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
+    // The speculative schedule needs the sequential monomer order, N >= 4 and two padding slots.
+    // PT_B200_SWEEP=serial forces the serial-schedule kernel (A/B measurements and tests).
+    const char* forced = getenv("PT_B200_SWEEP");
+    const bool serial_forced = forced && strcmp(forced, "serial") == 0;
+    int ni = -1;
+    if (d.select_mode == PT_SEQUENTIAL && d.N >= 4 && !serial_forced)
+      ni = precision == PT_F32 ? pt_spec_find_f32(L, (d.N + 2 + L - 1) / L) : pt_spec_find_f64(L, (d.N + 2 + L - 1) / L);
+    if (ni >= 0) {
+      pl.kind = PT_K_SPEC;
+      pl.ni = ni;
+      pl.Ns = ni > 0 ? ni * L : round_up(d.N + 2, L);
+    } else {
+      const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
+      if (!v) return cudaErrorInvalidValue;
+      pl.kind = PT_K_GROUP;
+      pl.ni = v->NI;
+      pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
+    }
     // chains of one warp must start in different banks: stride = L (mod Q) words, where Q words
     // span all 32 banks (fp64: a warp's 8-byte loads go in two phases of 16 lanes, Q = 16)
     const int Q = 128 / real_bytes;
@@ -480,6 +324,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.grid = (int)((d.C + pl.chains_per_cta - 1) / pl.chains_per_cta);
     pl.smem_bytes = pl.chains_per_cta * pl.sstride * real_bytes;
   } else {
+    pl.kind = PT_K_CTA;
     pl.ni = 0;
     pl.Ns = round_up(d.N, L);
     pl.sstride = 3 * pl.Ns;
@@ -489,11 +334,13 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.smem_bytes = pl.sstride * real_bytes;
   }
   if (pl.smem_bytes > 200 * 1024) return cudaErrorInvalidValue;
-  SweepFn fn = kernel_of(pl, precision);
-  if (!fn) return cudaErrorInvalidValue;
-  if (pl.smem_bytes > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem_bytes);
-    if (e != cudaSuccess) return e;
+  for (int trace = 0; trace < 2; ++trace) {
+    SweepFn fn = kernel_of(pl, precision, trace != 0);
+    if (!fn) return cudaErrorInvalidValue;
+    if (pl.smem_bytes > 48 * 1024) {
+      cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem_bytes);
+      if (e != cudaSuccess) return e;
+    }
   }
   *plan = pl;
   return cudaSuccess;
@@ -502,7 +349,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
 cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, uint32_t t0, int n_sweeps,
                             cudaStream_t stream)
 {
-  SweepFn fn = kernel_of(pl, precision);
+  SweepFn fn = kernel_of(pl, precision, d.tr_move != nullptr);
   if (!fn) return cudaErrorInvalidValue;
   fn<<<dim3(pl.grid), dim3(pl.threads), pl.smem_bytes, stream>>>(d, pl, t0, n_sweeps);
   return cudaGetLastError();
