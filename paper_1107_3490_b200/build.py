@@ -17,7 +17,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpt_b200.so"
-SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_sweep_spec_f64.cu", "pt_sweep_spec_f32.cu", "pt_peak.cu"]
+SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo", "--threads", "0",

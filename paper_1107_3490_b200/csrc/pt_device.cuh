@@ -32,6 +32,10 @@ __device__ __forceinline__ uint4 pt_draw(uint2 key, uint32_t a, uint32_t b, uint
   return pt_philox4x32_10(make_uint4(a, b, e, (tag << 24) | i), key);
 }
 
+// 2/(2k+3), k = 0..9: the odd series of log m = 2 atanh(s) after factoring out 2 s (PtNum<double>::log_)
+__constant__ double kPtLogC[10] = {2.0 / 3.0,  2.0 / 5.0,  2.0 / 7.0,  2.0 / 9.0,  2.0 / 11.0,
+                                   2.0 / 13.0, 2.0 / 15.0, 2.0 / 17.0, 2.0 / 19.0, 2.0 / 21.0};
+
 // ---- word -> number, proposal, reciprocal, cutoff test, per precision.
 // Every random value is exactly representable, so the proposal is bit-reproducible.
 template <typename Real> struct PtNum;
@@ -63,6 +67,8 @@ template <> struct PtNum<double> {
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
   }
+  // r2 < rc2, false for NaN; on the fp64 pipe (one DSETP instead of two ISETP on the half-rate ALU pipe)
+  static __device__ __forceinline__ bool inside(double r2, double rc2) { return r2 < rc2; }
   // the seed of rcp() alone, and whether it needs the Newton step
   static constexpr bool kNewton = true;
   static __device__ __forceinline__ double rcp_seed(double d)
@@ -70,6 +76,27 @@ template <> struct PtNum<double> {
     double x;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
     return x;
+  }
+  // Reciprocal seed of r2 if (j != m and r2 < rc2), else +0; cnt += delta in the first case.  One
+  // predicate from DSETP (fp64 pipe) drives a predicated MUFU and a predicated add: nothing is selected.
+  template <int DELTA>
+  static __device__ __forceinline__ double seed_if_inside(double r2, double rc2, int j, int m, int& cnt)
+  {
+    double x;
+    asm("{\n\t.reg .pred q, p;\n\t"
+        "setp.ne.s32 q, %4, %5;\n\t"
+        "setp.lt.and.f64 p, %2, %3, q;\n\t"
+        "mov.f64 %0, 0d0000000000000000;\n\t"
+        "@p rcp.approx.ftz.f64 %0, %2;\n\t"
+        "@p add.s32 %1, %1, %6;\n\t}"
+        : "=&d"(x), "+r"(cnt)
+        : "d"(r2), "d"(rc2), "r"(j), "r"(m), "n"(DELTA));
+    return x;
+  }
+  // keep ? x : +0 for a reciprocal seed x (its low word is zero): one integer select
+  static __device__ __forceinline__ double seed_or_zero(double x, bool keep)
+  {
+    return __hiloint2double(keep ? __double2hiint(x) : 0, __double2loint(x));
   }
   // r2 < rc2 for r2 >= 0 (or NaN), decided on the integer pipe: the bit patterns of non-negative
   // doubles are ordered like the numbers; NaN and anything with the sign bit set compare false.
@@ -92,15 +119,6 @@ template <> struct PtNum<double> {
     x = __hiloint2double(inside ? __double2hiint(x) : 0, __double2loint(x));
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
-  }
-  // Eq. (1) literally: E_LJ(min(r, r_c)).  Returns r2 if it lies below rc2 and `keep` holds, else
-  // rc2; compare and select on the integer pipe (bit patterns of non-negative doubles are ordered
-  // like the numbers; NaN and negative values compare false and clamp).
-  static __device__ __forceinline__ double clamp_below(double r2, double rc2, bool keep)
-  {
-    const bool in = below(r2, rc2) && keep;
-    return __hiloint2double(in ? __double2hiint(r2) : __double2hiint(rc2),
-                            in ? __double2loint(r2) : __double2loint(rc2));
   }
   // sqrt(a) for a normal a > 0, branch-free so that it can be scheduled between the pair terms:
   // y = MUFU.RSQ64H seed (relative error eps < 2^-19), g = a y, r = (1 - a y^2)/2, and
@@ -127,16 +145,11 @@ template <> struct PtNum<double> {
     const double f = m - 1.0;
     const double s = f * rcp(m + 1.0);
     const double z = s * s;
-    double p = 2.0 / 21.0;
-    p = fma(p, z, 2.0 / 19.0);
-    p = fma(p, z, 2.0 / 17.0);
-    p = fma(p, z, 2.0 / 15.0);
-    p = fma(p, z, 2.0 / 13.0);
-    p = fma(p, z, 2.0 / 11.0);
-    p = fma(p, z, 2.0 / 9.0);
-    p = fma(p, z, 2.0 / 7.0);
-    p = fma(p, z, 2.0 / 5.0);
-    p = fma(p, z, 2.0 / 3.0);
+    // coefficients come from the constant bank as the DFMA's third operand (as immediates they cost
+    // two UMOV per coefficient and step)
+    double p = kPtLogC[9];
+#pragma unroll
+    for (int q = 8; q >= 0; --q) p = fma(p, z, kPtLogC[q]);
     const double logm = fma(s, p * z, s + s);
     const double de = (double)e;
     return fma(de, 0x1.62e42fefa39efp-1, fma(de, 0x1.abc9e3b39803fp-56, logm));
@@ -162,8 +175,17 @@ template <> struct PtNum<float> {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return x;
   }
+  static __device__ __forceinline__ bool inside(float r2, float rc2) { return r2 < rc2; }
   static constexpr bool kNewton = false;
   static __device__ __forceinline__ float rcp_seed(float d) { return rcp(d); }
+  static __device__ __forceinline__ float seed_or_zero(float x, bool keep) { return keep ? x : 0.0f; }
+  template <int DELTA>
+  static __device__ __forceinline__ float seed_if_inside(float r2, float rc2, int j, int m, int& cnt)
+  {
+    const bool in = j != m && r2 < rc2;
+    cnt += in ? DELTA : 0;
+    return in ? rcp(r2) : 0.0f;
+  }
   static __device__ __forceinline__ bool below(float r2, float rc2) { return r2 < rc2; }
   static __device__ __forceinline__ float keep_or_far(float v, bool keep)
   {
@@ -174,10 +196,6 @@ template <> struct PtNum<float> {
     float x;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return inside ? x : 0.0f;
-  }
-  static __device__ __forceinline__ float clamp_below(float r2, float rc2, bool keep)
-  {
-    return (r2 < rc2 && keep) ? r2 : rc2;
   }
   static __device__ __forceinline__ float sqrt_(float v) { return sqrtf(v); }
   // the paper's fp32 kernels use the fast-math intrinsics (__logf)
@@ -190,9 +208,9 @@ template <> struct PtNum<float> {
 // The sums accumulate u (A u - B) with u = 0 for the pairs outside the cutoff, and count the pairs
 // inside; the caller subtracts C * count once per sum.
 template <typename Real> struct PtLJ {
-  Real A, nB, C, rc2;
+  Real A, nB, C, rc2, c;   // c = B / A = sigma^-6
   __device__ __forceinline__ explicit PtLJ(const PtDev& d)
-      : A((Real)d.ljA), nB((Real)-d.ljB), C((Real)d.ljC), rc2((Real)d.rc2)
+      : A((Real)d.ljA), nB((Real)-d.ljB), C((Real)d.ljC), rc2((Real)d.rc2), c((Real)(d.ljB / d.ljA))
   {
   }
   // acc += u (A u - B) for one squared distance; returns whether it lies inside the cutoff
@@ -203,15 +221,6 @@ template <typename Real> struct PtLJ {
     const Real u = inv * inv * inv;
     acc = fma(u, fma(A, u, nB), acc);
     return inside;
-  }
-  // acc += u (A u - B) at min(r2, rc2), or at rc2 if !keep: every call adds a term, the ones outside
-  // the cutoff (and the masked ones) add the constant E_LJ(r_c), which cancels between the sum over
-  // new and the sum over old distances because both have the same number of terms.
-  __device__ __forceinline__ void addc(Real r2, bool keep, Real& acc) const
-  {
-    const Real inv = PtNum<Real>::rcp(PtNum<Real>::clamp_below(r2, rc2, keep));
-    const Real u = inv * inv * inv;
-    acc = fma(u, fma(A, u, nB), acc);
   }
 };
 

@@ -55,20 +55,12 @@ struct PtLaunch {
   int sstride;         // shared-memory stride between chains, in Reals
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
-  int kind;            // PT_K_GROUP, PT_K_SPEC or PT_K_CTA
+  int kind;            // PT_K_GROUP or PT_K_CTA
 };
 
-enum { PT_K_GROUP = 0, PT_K_SPEC = 1, PT_K_CTA = 2 };
+enum { PT_K_GROUP = 0, PT_K_CTA = 2 };
 
 typedef void (*PtSweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
-
-// pt_sweep_spec_f64.cu / pt_sweep_spec_f32.cu: the speculative kernel's instantiations.
-// find: the unrolled iteration count NI (0 = run-time loop) of the variant with L lanes that covers
-// `ni_needed` partner iterations, or -1.
-int pt_spec_find_f64(int L, int ni_needed);
-int pt_spec_find_f32(int L, int ni_needed);
-PtSweepFn pt_spec_kernel_f64(int L, int NI, bool trace);
-PtSweepFn pt_spec_kernel_f32(int L, int NI, bool trace);
 
 // pt_sweep.cu
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan);

@@ -10,12 +10,98 @@
 // recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
 // long chains, and with the local Delta-E of Eq. (5) instead of the full sum.
 #include <math.h>
-#include <stdlib.h>
-#include <string.h>
 
 #include "pt_sweep_common.cuh"
 
 namespace {
+
+// A3 for CNT partner iterations at once (iterations BEGIN .. BEGIN+CNT-1 of this lane), written stage
+// by stage across the partners: every stage holds CNT or 2 CNT independent fp64 instructions, so that
+// a dependent instruction is not issued within the 8-cycle DFMA latency of its producer (written
+// partner by partner, ptxas kept one or two chains in flight).  Pairs inside the cutoff add
+// A u (u - c) - C with u = 1/r^6, c = B/A (Eq. 1-2); the others, and the moved monomer itself, get a
+// zero reciprocal seed, which stays zero through the Newton step and adds exactly nothing.  The
+// cutoff test is one DSETP (fp64 pipe) with the "not myself" mask as its predicate input, the mask
+// one integer select, the count of inside pairs one predicated add.  A and C are applied once per
+// step by the caller.  The new squared distance follows from the old one:
+// |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
+template <typename Real, int L, int BEGIN, int CNT>
+__device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
+                                           Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real (&en)[4],
+                                           Real (&eo)[4], int& cnt)
+{
+  Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) X.get(lig + (BEGIN + u) * L, bx[u], by[u], bz[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) { bx[u] = xo - bx[u]; by[u] = yo - by[u]; bz[u] = zo - bz[u]; }
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = bx[u] * bx[u];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = fma(by[u], by[u], ro[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = fma(bz[u], bz[u], ro[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + dd;
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdz, bz[u], rn[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdy, by[u], rn[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdx, bx[u], rn[u]);
+  Real dv[2 * CNT], xv[2 * CNT], ev[2 * CNT];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) {
+    const int j = lig + (BEGIN + u) * L;
+    dv[2 * u] = ro[u];
+    dv[2 * u + 1] = rn[u];
+    xv[2 * u] = PtNum<Real>::template seed_if_inside<-1>(ro[u], lj.rc2, j, m, cnt);
+    xv[2 * u + 1] = PtNum<Real>::template seed_if_inside<1>(rn[u], lj.rc2, j, m, cnt);
+  }
+  if (PtNum<Real>::kNewton) {
+#pragma unroll
+    for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(-dv[v], xv[v], (Real)1);
+#pragma unroll
+    for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(ev[v], ev[v], ev[v]);
+#pragma unroll
+    for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(xv[v], ev[v], xv[v]);
+  }
+#pragma unroll
+  for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] * xv[v];
+#pragma unroll
+  for (int v = 0; v < 2 * CNT; ++v) xv[v] = ev[v] * xv[v];          // u = 1/r^6
+#pragma unroll
+  for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] - lj.c;
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) {
+    eo[(BEGIN + u) & 3] = fma(xv[2 * u], ev[2 * u], eo[(BEGIN + u) & 3]);
+    en[(BEGIN + u) & 3] = fma(xv[2 * u + 1], ev[2 * u + 1], en[(BEGIN + u) & 3]);
+  }
+}
+
+// The whole partner loop of NI > 0 iterations in groups of four (the last group takes the rest):
+// returns this lane's share of Delta E_LJ.
+template <typename Real, int L, int NI>
+__device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
+                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd)
+{
+  Real en[4] = {(Real)0, (Real)0, (Real)0, (Real)0}, eo[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
+  int cnt = 0;
+#define PT_PG(B, C) pair_group<Real, L, B, C>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt)
+  if (NI <= 7) {
+    PT_PG(0, (NI <= 7 ? NI : 1));
+  } else if (NI <= 11) {
+    PT_PG(0, 4);
+    PT_PG(4, (NI > 7 && NI <= 11 ? NI - 4 : 1));
+  } else {
+    static_assert(NI <= 15, "add a group");
+    PT_PG(0, 4);
+    PT_PG(4, 4);
+    PT_PG(8, (NI > 11 ? NI - 8 : 1));
+  }
+#undef PT_PG
+  return fma(lj.A, ((en[0] - eo[0]) + (en[1] - eo[1])) + ((en[2] - eo[2]) + (en[3] - eo[3])), -lj.C * (Real)cnt);
+}
 
 // ------------------------------------------------------------------------------------------
 // Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
@@ -23,7 +109,7 @@ namespace {
 // NI > 0: the partner loop has exactly NI iterations (Ns = NI * L) and is unrolled completely, so
 // that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
 // pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
-template <typename Real, int L, int NI>
+template <typename Real, int L, int NI, bool TRACE>
 __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
@@ -82,20 +168,17 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
       const Real bond = bonds_and_logu<Real>(d, lig, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
 
       // A3: Delta E_LJ, lanes stride over partners (Eq. 1, 2)
-      Real en = (Real)0, eo = (Real)0;
-      int cnt = 0;
+      Real part;
       if (NI > 0) {
-#pragma unroll
-        for (int it = 0; it < NI; ++it) {
-          const int j = lig + it * L;
-          pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
-        }
+        part = pair_groups<Real, L, (NI > 0 ? NI : 1)>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd) + bond;
       } else {
+        Real en = (Real)0, eo = (Real)0;
+        int cnt = 0;
 #pragma unroll 2
         for (int j = lig; j < Ns; j += L)
           pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
+        part = fma(-lj.C, (Real)cnt, en - eo) + bond;
       }
-      const Real part = fma(-lj.C, (Real)cnt, en - eo) + bond;
       const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
       const Real logu = __shfl_sync(0xffffffffu, lg, g * L + 4);
 
@@ -108,8 +191,10 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
       // A7: commit
       if (lig == 0) {
         if (accept) X.set(m, xn, yn, zn);
-        if (d.tr_move && c.active && (long long)t < d.cap_sweeps)
-          d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
+        if (TRACE) {   // test support (pt_set_trace): a separate instantiation, the timed one has no branch here
+          if (d.tr_move && c.active && (long long)t < d.cap_sweeps)
+            d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
+        }
       }
       if (accept) { c.erun += (double)dE; c.acc++; }
       c.brej += bond_broken ? 1u : 0u;
@@ -226,10 +311,12 @@ typedef PtSweepFn SweepFn;
 
 struct SweepVariant {
   int L, NI;
-  SweepFn f64, f32;
+  SweepFn f64[2], f32[2];   // [0] timed, [1] with the decision trace
 };
 
-#define PT_VARIANT(L, NI) { L, NI, k_sweep_group<double, L, NI>, k_sweep_group<float, L, NI> }
+#define PT_VARIANT(L, NI)                                                              \
+  { L, NI, { k_sweep_group<double, L, NI, false>, k_sweep_group<double, L, NI, true> }, \
+    { k_sweep_group<float, L, NI, false>, k_sweep_group<float, L, NI, true> } }
 // Unrolled instantiations (NI = partner-loop iterations); NI = 0 is the run-time loop of the same
 // lane count and must come last within its L.
 const SweepVariant kVariants[] = {
@@ -249,10 +336,8 @@ const SweepVariant* find_variant(int L, int ni_needed)
 SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
-  if (pl.kind == PT_K_SPEC)
-    return precision == PT_F32 ? pt_spec_kernel_f32(pl.lanes, pl.ni, trace) : pt_spec_kernel_f64(pl.lanes, pl.ni, trace);
   for (const SweepVariant& v : kVariants)
-    if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32 : v.f64;
+    if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
   return nullptr;
 }
 
@@ -287,24 +372,11 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   pl.lanes = L;
   if (L <= 32) {
     const int G = 32 / L;
-    // The speculative schedule needs the sequential monomer order, N >= 4 and two padding slots.
-    // PT_B200_SWEEP=serial forces the serial-schedule kernel (A/B measurements and tests).
-    const char* forced = getenv("PT_B200_SWEEP");
-    const bool serial_forced = forced && strcmp(forced, "serial") == 0;
-    int ni = -1;
-    if (d.select_mode == PT_SEQUENTIAL && d.N >= 4 && !serial_forced)
-      ni = precision == PT_F32 ? pt_spec_find_f32(L, (d.N + 2 + L - 1) / L) : pt_spec_find_f64(L, (d.N + 2 + L - 1) / L);
-    if (ni >= 0) {
-      pl.kind = PT_K_SPEC;
-      pl.ni = ni;
-      pl.Ns = ni > 0 ? ni * L : round_up(d.N + 2, L);
-    } else {
-      const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
-      if (!v) return cudaErrorInvalidValue;
-      pl.kind = PT_K_GROUP;
-      pl.ni = v->NI;
-      pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
-    }
+    const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
+    if (!v) return cudaErrorInvalidValue;
+    pl.kind = PT_K_GROUP;
+    pl.ni = v->NI;
+    pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
     // chains of one warp must start in different banks: stride = L (mod Q) words, where Q words
     // span all 32 banks (fp64: a warp's 8-byte loads go in two phases of 16 lanes, Q = 16)
     const int Q = 128 / real_bytes;
