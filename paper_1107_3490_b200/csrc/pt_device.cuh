@@ -56,6 +56,9 @@ template <> struct PtNum<double> {
   {
     return __dadd_rn(x, __dmul_rn(d, s));
   }
+  // the same in two calls: delta = scale(d, s), x' = shift(x, delta)
+  static __device__ __forceinline__ double scale(double d, double s) { return __dmul_rn(d, s); }
+  static __device__ __forceinline__ double shift(double x, double delta) { return __dadd_rn(x, delta); }
   // 1/d for finite d > 0: MUFU.RCP64H seed (relative error < 2^-19.9 measured on B200) and one
   // cubic Newton step x (1 + e + e^2), e = 1 - d x  ->  relative error e^3 < 2^-59 before the
   // final rounding; measured worst case 2 ulp.  3 fp64-pipe instructions instead of the ~9 of an
@@ -169,6 +172,8 @@ template <> struct PtNum<float> {
   {
     return __fadd_rn(x, __fmul_rn(d, s));
   }
+  static __device__ __forceinline__ float scale(float d, float s) { return __fmul_rn(d, s); }
+  static __device__ __forceinline__ float shift(float x, float delta) { return __fadd_rn(x, delta); }
   static __device__ __forceinline__ float rcp(float d)
   {
     float x;

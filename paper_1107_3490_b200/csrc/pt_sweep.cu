@@ -15,6 +15,48 @@
 
 namespace {
 
+// A2 for eight steps at once.  All lanes of a chain would draw the same Philox block; instead lane l
+// (mod 8) draws the block of step g0 + l, converts it to the displacement (width * s, one rounding,
+// DESIGN.md R7) and the acceptance uniform, and every step fetches its four numbers with shuffles:
+// 1/8 of the integer work per step.  Steps are numbered g = sweep * N + k within the launch.
+template <typename Real> struct DrawBlock {
+  Real dx, dy, dz, u;
+  int m;
+};
+
+template <typename Real>
+__device__ __forceinline__ DrawBlock<Real> draw_block(const ChainCtx& c, bool pick, int N, Real width, uint32_t t0,
+                                                      int g0, int lig)
+{
+  const int gl = g0 + (lig & 7);
+  const uint32_t k = (uint32_t)(gl % N), t = t0 + (uint32_t)(gl / N);
+  DrawBlock<Real> b;
+  b.m = (int)k;
+  if (pick) {   // "a random monomer of the chain is picked"
+    const uint4 wp = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
+    b.m = (int)__umulhi(wp.x, (uint32_t)N);
+  }
+  const uint4 w = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
+  b.dx = PtNum<Real>::scale(width, PtNum<Real>::sym(w.x));
+  b.dy = PtNum<Real>::scale(width, PtNum<Real>::sym(w.y));
+  b.dz = PtNum<Real>::scale(width, PtNum<Real>::sym(w.z));
+  b.u = PtNum<Real>::u01(w.w);
+  return b;
+}
+
+template <typename Real>
+__device__ __forceinline__ DrawBlock<Real> draw_fetch(const DrawBlock<Real>& b, int g, unsigned gsh)
+{
+  const int src = (int)gsh + (g & 7);
+  DrawBlock<Real> r;
+  r.dx = __shfl_sync(0xffffffffu, b.dx, src);
+  r.dy = __shfl_sync(0xffffffffu, b.dy, src);
+  r.dz = __shfl_sync(0xffffffffu, b.dz, src);
+  r.u = __shfl_sync(0xffffffffu, b.u, src);
+  r.m = __shfl_sync(0xffffffffu, b.m, src);
+  return r;
+}
+
 // A3 for CNT partner iterations at once (iterations BEGIN .. BEGIN+CNT-1 of this lane), written stage
 // by stage across the partners: every stage holds CNT or 2 CNT independent fp64 instructions, so that
 // a dependent instruction is not issued within the 8-cycle DFMA latency of its producer (written
@@ -141,23 +183,25 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
   const unsigned bond_lanes = 3u << (g * L);   // roles 0, 1 of this group: the new bonds
   const double nbeta = -c.beta;
 
-  Proposal<Real> nx = draw_proposal<Real>(c, pick, N, 0u, t0);
+  const unsigned gsh = (unsigned)(g * L);
+  DrawBlock<Real> blk = draw_block<Real>(c, pick, N, width, t0, 0, lig);
+  DrawBlock<Real> nx = draw_fetch<Real>(blk, 0, gsh);
+  int gstep = 0;   // step number within the launch
   for (int sw = 0; sw < n_sweeps; ++sw) {
     const uint32_t t = t0 + (uint32_t)sw;
     for (int k = 0; k < N; ++k) {
-      // A2: this step's proposal was drawn one step ahead; draw the next one now so that the
-      // integer work overlaps the fp64 work below
-      const Proposal<Real> p = nx;
-      {
-        const bool last = k + 1 == N;
-        nx = draw_proposal<Real>(c, pick, N, last ? 0u : (uint32_t)(k + 1), last ? t + 1u : t);
-      }
+      // A2: this step's numbers were fetched one step ahead; fetch the next ones now (and draw the
+      // next eight blocks when they are used up) so that the shuffles overlap the fp64 work below
+      const DrawBlock<Real> p = nx;
+      ++gstep;
+      if ((gstep & 7) == 0) blk = draw_block<Real>(c, pick, N, width, t0, gstep, lig);
+      nx = draw_fetch<Real>(blk, gstep, gsh);
       const int m = p.m;
       Real xo, yo, zo;
       X.get(m, xo, yo, zo);
-      const Real xn = PtNum<Real>::propose(xo, width, p.sx);
-      const Real yn = PtNum<Real>::propose(yo, width, p.sy);
-      const Real zn = PtNum<Real>::propose(zo, width, p.sz);
+      const Real xn = PtNum<Real>::shift(xo, p.dx);
+      const Real yn = PtNum<Real>::shift(yo, p.dy);
+      const Real zn = PtNum<Real>::shift(zo, p.dz);
       const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
       const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
       const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
@@ -188,15 +232,14 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
       // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
       const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
 
-      // A7: commit
-      if (lig == 0) {
-        if (accept) X.set(m, xn, yn, zn);
-        if (TRACE) {   // test support (pt_set_trace): a separate instantiation, the timed one has no branch here
-          if (d.tr_move && c.active && (long long)t < d.cap_sweeps)
-            d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
-        }
+      // A7: commit (branch-free: one predicated store pair, selects for the bookkeeping)
+      if (accept && lig == 0) X.set(m, xn, yn, zn);
+      if (TRACE) {   // test support (pt_set_trace): a separate instantiation, the timed one has no branch here
+        if (lig == 0 && d.tr_move && c.active && (long long)t < d.cap_sweeps)
+          d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
       }
-      if (accept) { c.erun += (double)dE; c.acc++; }
+      c.erun += accept ? (double)dE : 0.0;
+      c.acc += accept ? 1u : 0u;
       c.brej += bond_broken ? 1u : 0u;
       __syncwarp();
     }
