@@ -36,7 +36,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12     # 37.2: 148 SMs x 64 fp
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 * 1e-12    # 74.4
 # fp64-pipe warp instructions the sweep kernel issues per attempted move at the default mapping of
 # config 5, counted in the SASS of the shipped kernel; used for pipe_frac.
-SWEEP_DRAM_TRAFFIC = 12.8e6       # dram read+write bytes per sweep launch of config 5 fp64, ncu --set full (profiles/r01_*_ncu_full.md)
+SWEEP_DRAM_TRAFFIC = 12.8e6       # dram read+write bytes per sweep launch of config 5 fp64, ncu --set full (profiles/r01_sweep_final_ncu_full.md)
 
 
 def parse_args():
