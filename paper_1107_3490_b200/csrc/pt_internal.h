@@ -56,6 +56,7 @@ struct PtLaunch {
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
   int kind;            // PT_K_GROUP or PT_K_CTA
+  int stagger;         // start delay in cycles per rank of a warp on its sub-partition (0 = none)
 };
 
 enum { PT_K_GROUP = 0, PT_K_CTA = 2 };

@@ -10,6 +10,7 @@
 // recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
 // long chains, and with the local Delta-E of Eq. (5) instead of the full sum.
 #include <math.h>
+#include <stdlib.h>
 
 #include "pt_sweep_common.cuh"
 
@@ -57,6 +58,114 @@ __device__ __forceinline__ DrawBlock<Real> draw_fetch(const DrawBlock<Real>& b, 
   return r;
 }
 
+// A5 + the logarithm of A6 (same roles and arithmetic as bonds_and_logu) cut into LEVELS of mutually
+// independent instructions.  A warp issues in order: as one block of code these ~30 dependent fp64
+// levels run back to back at the full 8-cycle DFMA latency (the S of DESIGN.md section 7, about 40 %
+// of a one-warp step).  The pair groups call run<P, NPTS>() after each of their stages instead: one
+// dependent level per ~10 independent pair instructions.  The logarithm's series is evaluated by
+// Estrin's scheme (depth 4 instead of 10).
+template <typename Real> struct BondChain {
+  static constexpr int NLEV = 31;
+  const PtDev& d;
+  const PtCoords<Real>& X;
+  int role, m, N;
+  Real xo, yo, zo, xn, yn, zn, u;
+  // results
+  Real bond, lg;
+  bool broke;
+  // intermediates
+  Real xb, yb, zb, dx, dy, dz, r2, r, q, gq;
+  Real y, g, h, rr, tt;
+  Real f, mp, x, e, sv, s2, z, z2, z4, z8, p01, p23, p45, p67, p89, q0, q1, pz, de;
+  bool isbond, isnew, in_range;
+
+  __device__ __forceinline__ BondChain(const PtDev& dev, const PtCoords<Real>& coords) : d(dev), X(coords) {}
+
+  template <int K> __device__ __forceinline__ void level()
+  {
+    if (K == 0) {
+      const int nb = (role & 1) ? m + 1 : m - 1;
+      isbond = role < 4 && nb >= 0 && nb < N;
+      isnew = role < 2;
+      X.get(isbond ? nb : m, xb, yb, zb);
+    }
+    if (K == 1) {
+      dx = (isnew ? xn : xo) - xb;
+      dy = (isnew ? yn : yo) - yb;
+      dz = (isnew ? zn : zo) - zb;
+    }
+    if (K == 2) r2 = dx * dx;
+    if (K == 3) r2 = fma(dy, dy, r2);
+    if (K == 4) { r2 = fma(dz, dz, r2); r2 = isbond ? r2 : (Real)(d.r0 * d.r0); }
+    if constexpr (sizeof(Real) == 8) {
+      // sqrt: MUFU.RSQ64H seed y, g = a y, r = (1 - a y^2)/2, sqrt a = g (1 + r + 3/2 r^2)
+      if (K == 5) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+      if (K == 6) { g = r2 * y; h = 0.5 * y; }
+      if (K == 7) rr = fma(-h, g, 0.5);
+      if (K == 8) tt = 1.5 * rr;
+      if (K == 9) tt = fma(tt, rr, rr);
+      if (K == 10) r = fma(g, tt, g);
+    } else {
+      if (K == 5) r = sqrtf(r2);
+    }
+    if (K == 11) q = r - (Real)d.r0;
+    if (K == 12) q = q * (Real)d.invR;
+    if (K == 13) gq = fma(-q, q, (Real)1);               // 1 - ((r - r0)/R)^2, Eq. (3)
+    if (K == 14) {
+      in_range = gq > (Real)0;                           // false for NaN as well
+      broke = isbond && isnew && !in_range;
+      gq = role == 4 ? u : ((isbond && in_range) ? gq : (Real)1);   // argument of the logarithm
+    }
+    if constexpr (sizeof(Real) == 8) {
+      // log v, v = 2^e m, m in [sqrt(1/2), sqrt(2)): log m = 2 atanh(s), s = (m-1)/(m+1) (PtNum<double>::log_)
+      if (K == 15) {
+        const int hi = __double2hiint(gq);
+        const int ex = (hi - 0x3fe6a09e) >> 20;
+        const double mm = __hiloint2double(hi - (ex << 20), __double2loint(gq));
+        de = (double)ex;
+        f = mm - 1.0;
+        mp = mm + 1.0;
+      }
+      if (K == 16) x = PtNum<double>::rcp_seed(mp);
+      if (K == 17) e = fma(-mp, x, 1.0);
+      if (K == 18) e = fma(e, e, e);
+      if (K == 19) x = fma(x, e, x);
+      if (K == 20) sv = f * x;
+      if (K == 21) { z = sv * sv; s2 = sv + sv; }
+      if (K == 22) {
+        p01 = fma(kPtLogC[1], z, kPtLogC[0]);
+        p23 = fma(kPtLogC[3], z, kPtLogC[2]);
+        p45 = fma(kPtLogC[5], z, kPtLogC[4]);
+        p67 = fma(kPtLogC[7], z, kPtLogC[6]);
+        p89 = fma(kPtLogC[9], z, kPtLogC[8]);
+        z2 = z * z;
+      }
+      if (K == 23) { q0 = fma(p23, z2, p01); q1 = fma(p67, z2, p45); z4 = z2 * z2; }
+      if (K == 24) { q0 = fma(q1, z4, q0); z8 = z4 * z4; }
+      if (K == 25) q0 = fma(p89, z8, q0);
+      if (K == 26) pz = q0 * z;
+      if (K == 27) lg = fma(sv, pz, s2);
+      if (K == 28) lg = fma(de, 0x1.abc9e3b39803fp-56, lg);
+      if (K == 29) lg = fma(de, 0x1.62e42fefa39efp-1, lg);
+    } else {
+      if (K == 15) lg = __logf(gq);
+    }
+    if (K == 30) bond = role < 4 ? (isnew ? (Real)d.feneC : (Real)-d.feneC) * lg : (Real)0;
+  }
+  template <int A, int B> __device__ __forceinline__ void range()
+  {
+    if constexpr (A < B) {
+      level<A>();
+      range<A + 1, B>();
+    }
+  }
+  // stage point P of NPTS
+  template <int P, int NPTS> __device__ __forceinline__ void run() { range<(P * NLEV) / NPTS, ((P + 1) * NLEV) / NPTS>(); }
+  __device__ __forceinline__ void run_all() { range<0, NLEV>(); }
+};
+
+constexpr int kGroupPoints = 14;   // stage points per pair group
+
 // A3 for CNT partner iterations at once (iterations BEGIN .. BEGIN+CNT-1 of this lane), written stage
 // by stage across the partners: every stage holds CNT or 2 CNT independent fp64 instructions, so that
 // a dependent instruction is not issued within the 8-cycle DFMA latency of its producer (written
@@ -67,30 +176,39 @@ __device__ __forceinline__ DrawBlock<Real> draw_fetch(const DrawBlock<Real>& b, 
 // one integer select, the count of inside pairs one predicated add.  A and C are applied once per
 // step by the caller.  The new squared distance follows from the old one:
 // |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
-template <typename Real, int L, int BEGIN, int CNT>
+template <typename Real, int L, int BEGIN, int CNT, int PBASE, int NPTS>
 __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real (&en)[4],
-                                           Real (&eo)[4], int& cnt)
+                                           Real (&eo)[4], int& cnt, BondChain<Real>& side)
 {
+#define PT_SIDE(n) side.template run<PBASE + (n), NPTS>()
   Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
 #pragma unroll
   for (int u = 0; u < CNT; ++u) X.get(lig + (BEGIN + u) * L, bx[u], by[u], bz[u]);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) { bx[u] = xo - bx[u]; by[u] = yo - by[u]; bz[u] = zo - bz[u]; }
+  PT_SIDE(0);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) ro[u] = bx[u] * bx[u];
+  PT_SIDE(1);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) ro[u] = fma(by[u], by[u], ro[u]);
+  PT_SIDE(2);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) ro[u] = fma(bz[u], bz[u], ro[u]);
+  PT_SIDE(3);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + dd;
+  PT_SIDE(4);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) rn[u] = fma(tdz, bz[u], rn[u]);
+  PT_SIDE(5);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) rn[u] = fma(tdy, by[u], rn[u]);
+  PT_SIDE(6);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) rn[u] = fma(tdx, bx[u], rn[u]);
+  PT_SIDE(7);
   Real dv[2 * CNT], xv[2 * CNT], ev[2 * CNT];
 #pragma unroll
   for (int u = 0; u < CNT; ++u) {
@@ -100,46 +218,56 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
     xv[2 * u] = PtNum<Real>::template seed_if_inside<-1>(ro[u], lj.rc2, j, m, cnt);
     xv[2 * u + 1] = PtNum<Real>::template seed_if_inside<1>(rn[u], lj.rc2, j, m, cnt);
   }
+  PT_SIDE(8);
   if (PtNum<Real>::kNewton) {
 #pragma unroll
     for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(-dv[v], xv[v], (Real)1);
+    PT_SIDE(9);
 #pragma unroll
     for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(ev[v], ev[v], ev[v]);
+    PT_SIDE(10);
 #pragma unroll
     for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(xv[v], ev[v], xv[v]);
   }
 #pragma unroll
   for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] * xv[v];
+  PT_SIDE(11);
 #pragma unroll
   for (int v = 0; v < 2 * CNT; ++v) xv[v] = ev[v] * xv[v];          // u = 1/r^6
+  PT_SIDE(12);
 #pragma unroll
   for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] - lj.c;
+  PT_SIDE(13);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) {
     eo[(BEGIN + u) & 3] = fma(xv[2 * u], ev[2 * u], eo[(BEGIN + u) & 3]);
     en[(BEGIN + u) & 3] = fma(xv[2 * u + 1], ev[2 * u + 1], en[(BEGIN + u) & 3]);
   }
+#undef PT_SIDE
 }
 
 // The whole partner loop of NI > 0 iterations in groups of four (the last group takes the rest):
 // returns this lane's share of Delta E_LJ.
 template <typename Real, int L, int NI>
 __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
-                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd)
+                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
+                                            BondChain<Real>& side)
 {
+  constexpr int P = kGroupPoints;
   Real en[4] = {(Real)0, (Real)0, (Real)0, (Real)0}, eo[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
   int cnt = 0;
-#define PT_PG(B, C) pair_group<Real, L, B, C>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt)
+#define PT_PG(B, C, PB, NP) \
+  pair_group<Real, L, B, C, PB, NP>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt, side)
   if (NI <= 7) {
-    PT_PG(0, (NI <= 7 ? NI : 1));
+    PT_PG(0, (NI <= 7 ? NI : 1), 0, P);
   } else if (NI <= 11) {
-    PT_PG(0, 4);
-    PT_PG(4, (NI > 7 && NI <= 11 ? NI - 4 : 1));
+    PT_PG(0, 4, 0, 2 * P);
+    PT_PG(4, (NI > 7 && NI <= 11 ? NI - 4 : 1), P, 2 * P);
   } else {
     static_assert(NI <= 15, "add a group");
-    PT_PG(0, 4);
-    PT_PG(4, 4);
-    PT_PG(8, (NI > 11 ? NI - 8 : 1));
+    PT_PG(0, 4, 0, 3 * P);
+    PT_PG(4, 4, P, 3 * P);
+    PT_PG(8, (NI > 11 ? NI - 8 : 1), 2 * P, 3 * P);
   }
 #undef PT_PG
   return fma(lj.A, ((en[0] - eo[0]) + (en[1] - eo[1])) + ((en[2] - eo[2]) + (en[3] - eo[3])), -lj.C * (Real)cnt);
@@ -178,6 +306,15 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
   }
   __syncwarp();
 
+  // Warps w and w + 4 of a CTA share an SM sub-partition and run the same code: started together they
+  // stay in phase, both in the fp64-bound pair loop, then both in the latency-bound serial part of
+  // the step (period 2P + S).  Started half a step apart, the serial part of one hides under the
+  // pair loop of the other (period 2P).  See DESIGN.md section 7, "Phase stagger".
+  if (pl.stagger > 0 && warp >= 4) {
+    const long long until = clock64() + (long long)pl.stagger * (warp >> 2);
+    while (clock64() < until) { }
+  }
+
   const bool pick = d.select_mode == PT_RANDOM_PICK;
   const bool leader = (lig == 0) && c.active;
   const unsigned bond_lanes = 3u << (g * L);   // roles 0, 1 of this group: the new bonds
@@ -206,23 +343,25 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
       const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
       const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
 
-      // A5: bonds, and log u of A6
-      Real lg;
-      bool broke;
-      const Real bond = bonds_and_logu<Real>(d, lig, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
-
-      // A3: Delta E_LJ, lanes stride over partners (Eq. 1, 2)
+      // A5 (bonds, and log u of A6) rides along with A3 (Delta E_LJ, lanes stride over partners, Eq. 1, 2)
+      BondChain<Real> bc(d, X);
+      bc.role = lig; bc.m = m; bc.N = N;
+      bc.xo = xo; bc.yo = yo; bc.zo = zo; bc.xn = xn; bc.yn = yn; bc.zn = zn; bc.u = p.u;
       Real part;
       if (NI > 0) {
-        part = pair_groups<Real, L, (NI > 0 ? NI : 1)>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd) + bond;
+        part = pair_groups<Real, L, (NI > 0 ? NI : 1)>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
       } else {
+        bc.run_all();
         Real en = (Real)0, eo = (Real)0;
         int cnt = 0;
 #pragma unroll 2
         for (int j = lig; j < Ns; j += L)
           pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
-        part = fma(-lj.C, (Real)cnt, en - eo) + bond;
+        part = fma(-lj.C, (Real)cnt, en - eo);
       }
+      part += bc.bond;
+      const Real lg = bc.lg;
+      const bool broke = bc.broke;
       const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
       const Real logu = __shfl_sync(0xffffffffu, lg, g * L + 4);
 
@@ -401,13 +540,16 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   const long long smsp = 4ll * sms;
   int L = lanes_requested;
   if (L == 0) {
-    // Few long chains: one CTA per replica.  Otherwise the fewest lanes per chain that still give
-    // every SM sub-partition a warp: the serial part of a step (proposal, bonds, log u, decision)
-    // is one instruction stream shared by the 32/L chains of a warp.
+    // Few long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
+    // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
+    // sub-partition costs more than halving the lanes (measured: profiles/r01_paper_timing.md, the
+    // steps at 592 -> 593 and 1184 -> 1185 replicas).  With more than 4 chains per sub-partition there
+    // is no such choice: 8 lanes, the serial part of a step (proposal, bonds, log u, decision) is then
+    // one instruction stream shared by 4 chains.
     if (d.N >= 192 && (long long)d.C <= smsp) L = 128;
     else {
       L = 32;
-      while (L > 8 && ((long long)d.C * (L / 2) + 31) / 32 >= smsp && d.N > L / 2) L /= 2;
+      while (L > 8 && ((long long)d.C * L + 31) / 32 > smsp && d.N > L / 2) L /= 2;
       while (L > 8 && L / 2 >= d.N) L /= 2;
     }
   }
@@ -436,6 +578,9 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     }
     pl.threads = 32 * wpc;
     pl.chains_per_cta = G * wpc;
+    // phase stagger between the warps of a sub-partition: about the fp64 time of one partner loop
+    pl.stagger = wpc > 4 ? (int)(2.1 * (26.0 * (pl.Ns / L) + 70.0)) : 0;
+    if (const char* e = getenv("PT_B200_STAGGER")) pl.stagger = atoi(e);
     pl.grid = (int)((d.C + pl.chains_per_cta - 1) / pl.chains_per_cta);
     pl.smem_bytes = pl.chains_per_cta * pl.sstride * real_bytes;
   } else {

@@ -23,7 +23,7 @@ from . import binding as pt
 from . import synth
 
 N, SWEEPS, EVERY = 55, 4000, 1000
-NR = [1, 2, 4, 8, 16, 32, 64, 128, 148, 149, 256, 296, 297, 512, 592, 593, 1024, 1184, 1185, 2048, 4096]
+NR = [1, 2, 4, 8, 16, 32, 64, 128, 148, 149, 256, 296, 297, 512, 592, 593, 1024, 1184, 1185, 2048, 2368, 2369, 4096]
 
 
 def run_one(n_r: int, precision: int, reps: int):
