@@ -146,6 +146,15 @@ int pt_set_trace(pt_handle* h, int64_t cap_sweeps, int64_t cap_events, uint8_t* 
 /* Sweep and exchange-event counters since pt_init. */
 int pt_counters(const pt_handle* h, int64_t* t_sweeps, int64_t* x_events);
 
+/* Exact resume.  The random stream is keyed by (seed, ensemble, temperature
+ * index, sweep t, step k) and by (pair, event x), and pt_read returns conformations by temperature
+ * index, so a run is continued bit for bit by: pt_init(seeds, conformations read at the break) on
+ * any handle with the same parameters, then pt_set_counters(t, x) with the counters read at the
+ * break.  Statistics restart from zero (add them outside); the running energy is recomputed by
+ * Eq. (4), i.e. it may differ from the uninterrupted one in the last bits.  0 <= t, x < 2^32;
+ * PT_ESTATE before pt_init, PT_ERANGE outside the range. */
+int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
+
 /* How the sweep kernel is mapped: lanes per chain (as in pt_params.lanes, resolved), chains per
  * CTA, CTAs in the grid, dynamic shared memory bytes per CTA.  Any pointer may be NULL. */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,

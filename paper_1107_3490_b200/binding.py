@@ -24,7 +24,7 @@ _ERRNAMES = {-1: "PT_EINVAL", -2: "PT_ESTATE", -3: "PT_EBOND", -4: "PT_ENOMEM", 
 # every symbol include/pt_b200.h declares
 SYMBOLS = ("pt_workspace_bytes", "pt_create", "pt_create_with_workspace", "pt_destroy", "pt_init",
            "pt_sweeps", "pt_exchange", "pt_run", "pt_read", "pt_recompute_energy", "pt_reset_stats",
-           "pt_set_trace", "pt_counters", "pt_launch_info", "pt_kernel_launches", "pt_last_error",
+           "pt_set_trace", "pt_counters", "pt_set_counters", "pt_launch_info", "pt_kernel_launches", "pt_last_error",
            "pt_fma_peak")
 
 
@@ -78,6 +78,7 @@ def lib():
     L.pt_set_trace.argtypes = [hp, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
     L.pt_set_trace.restype = C.c_int
     L.pt_counters.argtypes = [hp, i64p, i64p]; L.pt_counters.restype = C.c_int
+    L.pt_set_counters.argtypes = [hp, C.c_int64, C.c_int64]; L.pt_set_counters.restype = C.c_int
     L.pt_launch_info.argtypes = [hp, i32p, i32p, i32p, i32p]; L.pt_launch_info.restype = C.c_int
     L.pt_kernel_launches.argtypes = [hp]; L.pt_kernel_launches.restype = C.c_int64
     L.pt_last_error.argtypes = [hp]; L.pt_last_error.restype = C.c_char_p
@@ -265,6 +266,9 @@ class ParallelTempering:
         t, x = C.c_int64(0), C.c_int64(0)
         _check(self._h, lib().pt_counters(self._h, C.byref(t), C.byref(x)))
         return t.value, x.value
+
+    def pt_set_counters(self, t_sweeps: int, x_events: int):
+        _check(self._h, lib().pt_set_counters(self._h, int(t_sweeps), int(x_events)))
 
     def pt_launch_info(self) -> dict:
         a, b, c, d = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)

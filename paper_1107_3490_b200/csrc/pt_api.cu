@@ -382,6 +382,17 @@ int pt_counters(const pt_handle* h, int64_t* t_sweeps, int64_t* x_events)
   return PT_OK;
 }
 
+int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events)
+{
+  if (!h) return PT_EINVAL;
+  if (!h->initialised) return fail(h, PT_ESTATE, "pt_set_counters before pt_init");
+  if (t_sweeps < 0 || x_events < 0 || t_sweeps > 0xFFFFFFFFll || x_events > 0xFFFFFFFFll)
+    return fail(h, PT_ERANGE, "counters must lie in [0, 2^32)");
+  h->t = t_sweeps;
+  h->x = x_events;
+  return PT_OK;
+}
+
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid, int32_t* smem_bytes)
 {
   if (!h) return PT_EINVAL;

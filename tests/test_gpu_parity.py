@@ -192,6 +192,41 @@ def test_reset_stats_and_resume():
     assert (b["move_counts"][..., 0] == 100 * wl.N).all()
 
 
+def test_exact_resume_from_read_state():
+    """pt_read at a break + pt_init + pt_set_counters on a fresh handle continues
+    the run bit for bit (coordinates, decisions, swap decisions), across an odd exchange parity."""
+    inp = synth.make_inputs(2)
+    wl = inp.workload
+    S = wl.exchange_every
+    p = pt.make_params(wl.N, wl.M, wl.E, nbins=0)
+    n1, n2 = 70, 50      # break after 7 exchange events: the next event has odd parity
+    with pt.ParallelTempering(p, inp.temperatures, inp.widths) as a:
+        a.pt_init(inp.seeds, inp.conformations)
+        a.pt_set_trace(n1 + n2, (n1 + n2) // S)
+        a.pt_run(n1 + n2, S)
+        full, ftr = a.pt_read(), a.trace()
+    with pt.ParallelTempering(p, inp.temperatures, inp.widths) as b:
+        b.pt_init(inp.seeds, inp.conformations)
+        b.pt_run(n1, S)
+        mid = b.pt_read()
+        t, x = b.pt_counters()
+    assert (t, x) == (n1, n1 // S)
+    with pt.ParallelTempering(p, inp.temperatures, inp.widths) as c:
+        c.pt_init(inp.seeds, mid["conformations"])
+        c.pt_set_counters(t, x)
+        c.pt_set_trace(n1 + n2, (n1 + n2) // S)
+        c.pt_run(n2, S)
+        res, rtr = c.pt_read(), c.trace()
+        assert c.pt_counters() == (n1 + n2, (n1 + n2) // S)
+    assert np.array_equal(res["conformations"].view(np.uint64), full["conformations"].view(np.uint64))
+    assert np.array_equal(rtr["move"][:, :, n1:], ftr["move"][:, :, n1:])
+    assert np.array_equal(rtr["swap"][:, n1 // S:], ftr["swap"][:, n1 // S:])
+    assert energy_close(res["energies"], full["energies"]).all()
+    with pytest.raises(pt.PtError):
+        with pt.ParallelTempering(p, inp.temperatures, inp.widths) as e:
+            e.pt_set_counters(1, 1)          # before pt_init
+
+
 def test_determinism_and_seed_locality():
     """Same seeds -> identical output; changing one ensemble's seed changes only that ensemble."""
     inp = synth.make_inputs(5, E=4)
