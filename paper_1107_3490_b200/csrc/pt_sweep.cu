@@ -10,7 +10,6 @@
 // recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
 // long chains, and with the local Delta-E of Eq. (5) instead of the full sum.
 #include <math.h>
-#include <stdlib.h>
 
 #include "pt_sweep_common.cuh"
 
@@ -505,7 +504,8 @@ const SweepVariant kVariants[] = {
     PT_VARIANT(8, 2),  PT_VARIANT(8, 4),  PT_VARIANT(8, 7),  PT_VARIANT(8, 10), PT_VARIANT(8, 13),
     PT_VARIANT(8, 0),
     PT_VARIANT(16, 1), PT_VARIANT(16, 2), PT_VARIANT(16, 4), PT_VARIANT(16, 7), PT_VARIANT(16, 0),
-    PT_VARIANT(32, 1), PT_VARIANT(32, 2), PT_VARIANT(32, 4), PT_VARIANT(32, 0),
+    PT_VARIANT(32, 1), PT_VARIANT(32, 2), PT_VARIANT(32, 4), PT_VARIANT(32, 7), PT_VARIANT(32, 10),
+    PT_VARIANT(32, 13), PT_VARIANT(32, 15), PT_VARIANT(32, 0),
 };
 
 const SweepVariant* find_variant(int L, int ni_needed)
@@ -540,13 +540,13 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   const long long smsp = 4ll * sms;
   int L = lanes_requested;
   if (L == 0) {
-    // Few long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
+    // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
     // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
     // sub-partition costs more than halving the lanes (measured: profiles/r01_paper_timing.md, the
     // steps at 592 -> 593 and 1184 -> 1185 replicas).  With more than 4 chains per sub-partition there
     // is no such choice: 8 lanes, the serial part of a step (proposal, bonds, log u, decision) is then
     // one instruction stream shared by 4 chains.
-    if (d.N >= 192 && (long long)d.C <= smsp) L = 128;
+    if (d.N > 15 * 32 && (long long)d.C <= smsp) L = 128;   // beyond the unrolled one-warp variants (15 iterations)
     else {
       L = 32;
       while (L > 8 && ((long long)d.C * L + 31) / 32 > smsp && d.N > L / 2) L /= 2;
@@ -580,7 +580,6 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.chains_per_cta = G * wpc;
     // phase stagger between the warps of a sub-partition: about the fp64 time of one partner loop
     pl.stagger = wpc > 4 ? (int)(2.1 * (26.0 * (pl.Ns / L) + 70.0)) : 0;
-    if (const char* e = getenv("PT_B200_STAGGER")) pl.stagger = atoi(e);
     pl.grid = (int)((d.C + pl.chains_per_cta - 1) / pl.chains_per_cta);
     pl.smem_bytes = pl.chains_per_cta * pl.sstride * real_bytes;
   } else {
