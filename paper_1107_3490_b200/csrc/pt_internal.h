@@ -55,11 +55,12 @@ struct PtLaunch {
   int sstride;         // shared-memory stride between chains, in Reals
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
-  int kind;            // PT_K_GROUP or PT_K_CTA
+  int sstride2;        // PT_K_MIXED: stride of the 10-lane chains
+  int kind;            // PT_K_GROUP, PT_K_MIXED or PT_K_CTA
   int stagger;         // start delay in cycles per rank of a warp on its sub-partition (0 = none)
 };
 
-enum { PT_K_GROUP = 0, PT_K_CTA = 2 };
+enum { PT_K_GROUP = 0, PT_K_MIXED = 1, PT_K_CTA = 2 };
 
 typedef void (*PtSweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
 

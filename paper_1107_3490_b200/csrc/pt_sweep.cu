@@ -227,6 +227,9 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
     PT_SIDE(10);
 #pragma unroll
     for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(xv[v], ev[v], xv[v]);
+  } else {   // fp32: the MUFU reciprocal is final; the serial stream still gets its two turns
+    PT_SIDE(9);
+    PT_SIDE(10);
   }
 #pragma unroll
   for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] * xv[v];
@@ -278,24 +281,27 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
 // NI > 0: the partner loop has exactly NI iterations (Ns = NI * L) and is unrolled completely, so
 // that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
 // pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
+// One warp's share of a sweep launch: G = 32 / L chains starting at slot `chain0`, coordinates at
+// `smem0` (stride `sstride` Reals between chains, Ns slots per coordinate array).  `delay`: cycles to
+// wait before the first step (phase stagger).
 template <typename Real, int L, int NI, bool TRACE>
-__global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
-                                                     const int n_sweeps)
+__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns, int chain0, int delay,
+                                           const uint32_t t0, const int n_sweeps)
 {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
   static_assert(L >= 8 && L <= 32, "lanes per chain");
   constexpr int G = 32 / L;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // lanes beyond G L (L = 10: lanes 30, 31) are ghosts: they repeat the last real lane and nobody reads them
+  const int lane = min((int)(threadIdx.x & 31), G * L - 1);
   const int g = lane / L, lig = lane % L;
-  const int cl = warp * G + g;
-  const int N = d.N, Ns = pl.Ns;
+  const int gbase = g * L;
+  const int N = d.N;
 
   ChainCtx c;
-  ctx_load(d, blockIdx.x * pl.chains_per_cta + cl, c);
+  ctx_load(d, chain0 + g, c);
   const Real width = (Real)d.width[c.i];
   const PtLJ<Real> lj(d);
 
-  const PtCoords<Real> X(reinterpret_cast<Real*>(smem_raw) + (size_t)cl * pl.sstride, Ns);
+  const PtCoords<Real> X(smem0 + (size_t)g * sstride, Ns);
 
   // A1: HBM -> shared memory; padding entries lie far outside every cutoff
   Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
@@ -305,21 +311,17 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
   }
   __syncwarp();
 
-  // Warps w and w + 4 of a CTA share an SM sub-partition and run the same code: started together they
-  // stay in phase, both in the fp64-bound pair loop, then both in the latency-bound serial part of
-  // the step (period 2P + S).  Started half a step apart, the serial part of one hides under the
-  // pair loop of the other (period 2P).  See DESIGN.md section 7, "Phase stagger".
-  if (pl.stagger > 0 && warp >= 4) {
-    const long long until = clock64() + (long long)pl.stagger * (warp >> 2);
+  if (delay > 0) {
+    const long long until = clock64() + (long long)delay;
     while (clock64() < until) { }
   }
 
   const bool pick = d.select_mode == PT_RANDOM_PICK;
   const bool leader = (lig == 0) && c.active;
-  const unsigned bond_lanes = 3u << (g * L);   // roles 0, 1 of this group: the new bonds
+  const unsigned bond_lanes = 3u << gbase;   // roles 0, 1 of this group: the new bonds
   const double nbeta = -c.beta;
 
-  const unsigned gsh = (unsigned)(g * L);
+  const unsigned gsh = (unsigned)gbase;
   DrawBlock<Real> blk = draw_block<Real>(c, pick, N, width, t0, 0, lig);
   DrawBlock<Real> nx = draw_fetch<Real>(blk, 0, gsh);
   int gstep = 0;   // step number within the launch
@@ -362,10 +364,10 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
       const Real lg = bc.lg;
       const bool broke = bc.broke;
       const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
-      const Real logu = __shfl_sync(0xffffffffu, lg, g * L + 4);
+      const Real logu = __shfl_sync(0xffffffffu, lg, gbase + 4);
 
       // A4: reduce; every lane of the group gets the same Delta E
-      const Real dE = group_sum<Real, L>(part);
+      const Real dE = group_sum<Real, L>(part, lig, gbase);
 
       // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
       const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
@@ -383,7 +385,7 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
     }
 
     // A8: measurement once per sweep
-    if (d.observables) measure_shape<Real, L>(c, N, lig, X);
+    if (d.observables) measure_shape<Real, L>(c, N, lig, gbase, X);
     if (leader) measure_energy(d, c, t);
   }
 
@@ -393,6 +395,42 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
     for (int j = lig; j < N; j += L) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
     if (lig == 0) ctx_store(d, c, n_sweeps);
   }
+}
+
+// Warps w and w + 4 of a CTA share an SM sub-partition and run the same code: started together they
+// stay in phase, both in the fp64-bound pair loop, then both in the latency-bound serial part of
+// the step (period 2P + S).  The second one therefore starts `stagger` cycles (about one partner
+// loop) late, so that its serial part can hide under the pair loop of the first.
+template <typename Real, int L, int NI, bool TRACE>
+__global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
+                                                     const int n_sweeps)
+{
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  constexpr int G = 32 / L;
+  const int warp = threadIdx.x >> 5;
+  sweep_warp<Real, L, NI, TRACE>(d, reinterpret_cast<Real*>(smem_raw) + (size_t)(warp * G) * pl.sstride, pl.sstride, pl.Ns,
+                                 blockIdx.x * pl.chains_per_cta + warp * G, pl.stagger * (warp >> 2), t0, n_sweeps);
+}
+
+// Mixed mapping against wave quantisation (the paper's staircase): when the chains
+// per sub-partition lie between 4 and 7, uniform 4-chain warps leave sub-partitions with two warps
+// (8 chains) next to sub-partitions with one.  Here every sub-partition gets 7 chains: one warp of
+// 4 chains x 8 lanes (13 partner iterations) and one warp of 3 chains x 10 lanes (10 iterations, lanes
+// 30, 31 idle), 28 chains per CTA of 8 warps.  Instantiated for 97 <= N <= 100 (13 x 8 and 10 x 10 slots).
+template <typename Real, bool TRACE>
+__global__ void __launch_bounds__(256, 1) k_sweep_mixed(const PtDev d, const PtLaunch pl, const uint32_t t0,
+                                                     const int n_sweeps)
+{
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Real* base = reinterpret_cast<Real*>(smem_raw);
+  const int warp = threadIdx.x >> 5;
+  const int cta0 = blockIdx.x * 28;
+  if (warp < 4)
+    sweep_warp<Real, 8, 13, TRACE>(d, base + (size_t)(warp * 4) * pl.sstride, pl.sstride, 104, cta0 + warp * 4, 0, t0,
+                                   n_sweeps);
+  else
+    sweep_warp<Real, 10, 10, TRACE>(d, base + (size_t)16 * pl.sstride + (size_t)((warp - 4) * 3) * pl.sstride2,
+                                    pl.sstride2, 100, cta0 + 16 + (warp - 4) * 3, pl.stagger, t0, n_sweeps);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -457,7 +495,7 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
         part += bonds_and_logu<Real>(d, lane, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
         if (lane == 4) s_logu[k & 1] = (double)lg;
       }
-      const Real wsum = group_sum<Real, 32>(part);
+      const Real wsum = group_sum<Real, 32>(part, lane, 0);
       if (lane == 0) red[k & 1][warp] = (double)wsum;
       const bool bond_broken = __syncthreads_or(broke ? 1 : 0) != 0;
       double dEd = red[k & 1][0];
@@ -477,7 +515,7 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
       __syncthreads();
     }
 
-    if (d.observables && warp == 0) measure_shape<Real, 32>(c, N, lane, X);
+    if (d.observables && warp == 0) measure_shape<Real, 32>(c, N, lane, 0, X);
     if (tid == 0) measure_energy(d, c, t);
   }
 
@@ -518,6 +556,10 @@ const SweepVariant* find_variant(int L, int ni_needed)
 SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
+  if (pl.kind == PT_K_MIXED) {
+    if (precision == PT_F32) return trace ? (SweepFn)k_sweep_mixed<float, true> : (SweepFn)k_sweep_mixed<float, false>;
+    return trace ? (SweepFn)k_sweep_mixed<double, true> : (SweepFn)k_sweep_mixed<double, false>;
+  }
   for (const SweepVariant& v : kVariants)
     if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
   return nullptr;
@@ -555,7 +597,24 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   }
   PtLaunch pl{};
   pl.lanes = L;
-  if (L <= 32) {
+  if (lanes_requested == 0 && L == 8 && d.N >= 97 && d.N <= 100 && (long long)d.C > 4 * smsp && (long long)d.C <= 7 * smsp) {
+    // between 4 and 7 chains per sub-partition: 4 + 3 chains on every one (k_sweep_mixed)
+    const int Q = 128 / real_bytes;
+    pl.kind = PT_K_MIXED;
+    pl.ni = 13;
+    pl.Ns = 104;
+    int ss = 3 * 104;
+    while (ss % Q != 8 % Q) ++ss;
+    pl.sstride = ss;
+    ss = 3 * 100;
+    while (ss % Q != 10 % Q) ++ss;
+    pl.sstride2 = ss;
+    pl.threads = 256;
+    pl.chains_per_cta = 28;
+    pl.stagger = 0;   // the two kinds of warp have different periods: a start delay changes nothing (measured)
+    pl.grid = (int)((d.C + 27) / 28);
+    pl.smem_bytes = (16 * pl.sstride + 12 * pl.sstride2) * real_bytes;
+  } else if (L <= 32) {
     const int G = 32 / L;
     const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
     if (!v) return cudaErrorInvalidValue;

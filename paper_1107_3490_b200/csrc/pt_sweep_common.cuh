@@ -7,11 +7,27 @@
 
 namespace {
 
-template <typename Real, int L> __device__ __forceinline__ Real group_sum(Real v)
+// Sum over the L lanes of a chain's group, returned to all of them.  lig = lane in group, gbase = first
+// lane of the group.  L a power of two: butterfly.  Otherwise (L = 10: three chains per warp, lanes
+// 30, 31 are ghosts that duplicate lane 29 and are never read): a tree padded to the next power of
+// two, then a broadcast from the group's first lane.
+template <typename Real, int L> __device__ __forceinline__ Real group_sum(Real v, int lig, int gbase)
 {
+  if ((L & (L - 1)) == 0) {
 #pragma unroll
-  for (int o = L / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
+    for (int o = L / 2; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+  }
+  int active = L;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    if (o < L) {
+      const Real w = __shfl_down_sync(0xffffffffu, v, o);
+      v += (lig < o && lig + o < active) ? w : (Real)0;
+      active = o < active ? o : active;
+    }
+  }
+  return __shfl_sync(0xffffffffu, v, gbase);
 }
 
 // Everything a chain carries through a launch besides its coordinates.
@@ -154,7 +170,7 @@ __device__ __forceinline__ Real bonds_and_logu(const PtDev& d, int role, int m, 
 
 // Eq. (8), and R_ee once per sweep; all lanes of the group take part.
 template <typename Real, int L>
-__device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const PtCoords<Real>& X)
+__device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, int gbase, const PtCoords<Real>& X)
 {
   double sx = 0.0, sy = 0.0, sz = 0.0;
   for (int j = lig; j < N; j += L) {
@@ -162,9 +178,9 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const
     X.get(j, x, y, z);
     sx += (double)x; sy += (double)y; sz += (double)z;
   }
-  sx = group_sum<double, L>(sx) / (double)N;
-  sy = group_sum<double, L>(sy) / (double)N;
-  sz = group_sum<double, L>(sz) / (double)N;
+  sx = group_sum<double, L>(sx, lig, gbase) / (double)N;
+  sy = group_sum<double, L>(sy, lig, gbase) / (double)N;
+  sz = group_sum<double, L>(sz, lig, gbase) / (double)N;
   double q = 0.0;
   for (int j = lig; j < N; j += L) {
     Real x, y, z;
@@ -172,7 +188,7 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, const
     const double dx = (double)x - sx, dy = (double)y - sy, dz = (double)z - sz;
     q += dx * dx + dy * dy + dz * dz;
   }
-  const double rg2 = group_sum<double, L>(q) / (double)N;
+  const double rg2 = group_sum<double, L>(q, lig, gbase) / (double)N;
   Real x0, y0, z0, x1, y1, z1;
   X.get(0, x0, y0, z0);
   X.get(N - 1, x1, y1, z1);
