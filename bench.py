@@ -36,6 +36,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 * 1e-12     # 37.2: 148 SMs x 64 fp
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 * 1e-12    # 74.4
 # fp64-pipe warp instructions the sweep kernel issues per attempted move at the default mapping of
 # config 5, counted in the SASS of the shipped kernel; used for pipe_frac.
+NCU_PIPE_FP64_PCT = 69.6
 SWEEP_DRAM_TRAFFIC = 12.8e6       # dram read+write bytes per sweep launch of config 5 fp64, ncu --set full (profiles/r01_sweep_final_ncu_full.md)
 
 
@@ -294,7 +295,10 @@ def run_ours(args, rank, world, local):
                 "peak_kind": f"measured {'fp32' if f32 else 'fp64'} FMA chain (pt_fma_peak), this run",
                 "peak_nominal": NOMINAL_FP32_TFLOPS if f32 else NOMINAL_FP64_TFLOPS,
                 "flops_per_pair_eval": FLOPS_PER_PAIR_EVAL,
-                "kernel_share_of_step": (k_s * (n_sweeps // S)) / (t_dev / args.steps) if world == 1 else None}
+                "kernel_share_of_step": (k_s * (n_sweeps // S)) / (t_dev / args.steps) if world == 1 else None,
+                # sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active of the committed ncu capture of this
+                # command (profiles/r01_sweep_final_ncu_full.md): the figure the 50 % target is read against
+                "ncu_pipe_fp64_pct": NCU_PIPE_FP64_PCT if (args.config == 5 and not f32 and args.lanes == 0) else None}
 
     # end to end through the C ABI with HOST buffers: pt_init (H2D) + pt_run + pt_read (D2H)
     e2e = None
@@ -335,6 +339,11 @@ def run_ours(args, rank, world, local):
         cpu_baseline = {"value": moves / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": f"first {ne} of {wl.E} ensembles ({ne * wl.M} chains), {ns} of {n_sweeps} sweeps, "
                                   f"exchange every {S}; {times[0]:.2f} s wall on {cores} threads"}
+        # the paper's convention is ONE core: a smaller sample on one thread
+        ns1 = max(S, ns // 4)
+        moves1, times1 = oracle_sample_run(inp, 1, ns1, 1)
+        cpu_baseline["one_thread"] = {"value": moves1 / times1[0], "unit": UNIT, "cores": 1,
+                                      "sample": f"first ensemble ({wl.M} chains), {ns1} sweeps; {times1[0]:.2f} s wall"}
     sim.pt_destroy()
     if rank != 0:
         return

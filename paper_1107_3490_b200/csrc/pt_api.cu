@@ -271,8 +271,10 @@ int pt_sweeps(pt_handle* h, int64_t n)
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_sweeps before pt_init");
   if (n < 0) return fail(h, PT_EINVAL, "n must be >= 0");
   if (h->t + n > 0xFFFFFFFFll) return fail(h, PT_ERANGE, "sweep counter would exceed 2^32 - 1");
+  // one launch numbers its steps 0 .. chunk N - 1 (+ 8 drawn ahead) in an int
+  const int64_t max_chunk = (2147483647ll - 16) / h->d.N;
   while (n > 0) {
-    const int chunk = (int)(n > (1 << 30) ? (1 << 30) : n);
+    const int chunk = (int)(n > max_chunk ? max_chunk : n);
     PT_CUDA(h, pt_launch_sweep(h->d, h->p.precision, h->plan, (uint32_t)h->t, chunk, h->stream));
     h->launches += 1;
     h->t += chunk;
