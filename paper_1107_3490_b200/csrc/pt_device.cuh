@@ -70,8 +70,6 @@ template <> struct PtNum<double> {
     const double e = fma(-d, x, 1.0);
     return fma(x, fma(e, e, e), x);
   }
-  // r2 < rc2, false for NaN; on the fp64 pipe (one DSETP instead of two ISETP on the half-rate ALU pipe)
-  static __device__ __forceinline__ bool inside(double r2, double rc2) { return r2 < rc2; }
   // the seed of rcp() alone, and whether it needs the Newton step
   static constexpr bool kNewton = true;
   static __device__ __forceinline__ double rcp_seed(double d)
@@ -80,8 +78,10 @@ template <> struct PtNum<double> {
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
     return x;
   }
-  // Reciprocal seed of r2 if (j != m and r2 < rc2), else +0; cnt += delta in the first case.  One
-  // predicate from DSETP (fp64 pipe) drives a predicated MUFU and a predicated add: nothing is selected.
+  // Reciprocal seed of r2 if (j != m and r2 < rc2), else +0; cnt += DELTA in the first case.  One
+  // predicate from a DSETP (fp64 pipe; "j != m" is its predicate input) masks the seed and drives a
+  // predicated add.  Written in PTX to keep that shape: ptxas emits MUFU.RCP64H + one FSEL on the seed's
+  // high word (the low word of a seed is zero anyway), where C++ source gave two ISETP, SEL and a move.
   template <int DELTA>
   static __device__ __forceinline__ double seed_if_inside(double r2, double rc2, int j, int m, int& cnt)
   {
@@ -95,11 +95,6 @@ template <> struct PtNum<double> {
         : "=&d"(x), "+r"(cnt)
         : "d"(r2), "d"(rc2), "r"(j), "r"(m), "n"(DELTA));
     return x;
-  }
-  // keep ? x : +0 for a reciprocal seed x (its low word is zero): one integer select
-  static __device__ __forceinline__ double seed_or_zero(double x, bool keep)
-  {
-    return __hiloint2double(keep ? __double2hiint(x) : 0, __double2loint(x));
   }
   // r2 < rc2 for r2 >= 0 (or NaN), decided on the integer pipe: the bit patterns of non-negative
   // doubles are ordered like the numbers; NaN and anything with the sign bit set compare false.
@@ -180,10 +175,8 @@ template <> struct PtNum<float> {
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(x) : "f"(d));
     return x;
   }
-  static __device__ __forceinline__ bool inside(float r2, float rc2) { return r2 < rc2; }
   static constexpr bool kNewton = false;
   static __device__ __forceinline__ float rcp_seed(float d) { return rcp(d); }
-  static __device__ __forceinline__ float seed_or_zero(float x, bool keep) { return keep ? x : 0.0f; }
   template <int DELTA>
   static __device__ __forceinline__ float seed_if_inside(float r2, float rc2, int j, int m, int& cnt)
   {
