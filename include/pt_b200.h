@@ -157,7 +157,7 @@ int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
 
 /* How the sweep kernel is mapped: lanes per chain (as in pt_params.lanes, resolved), chains per
  * CTA, CTAs in the grid, dynamic shared memory bytes per CTA.  Any pointer may be NULL.  With
- * lanes = 0 and between 4 and 7 chains per SM sub-partition (and 97 <= N <= 100) the library maps
+ * lanes = 0 and between 4 and 7 chains per SM sub-partition (and N in 51..56 or 97..100) the library maps
  * 4 chains x 8 lanes + 3 chains x 10 lanes on every sub-partition; it then reports 8 lanes and 28
  * chains per CTA. */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,

@@ -416,8 +416,9 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
 // per sub-partition lie between 4 and 7, uniform 4-chain warps leave sub-partitions with two warps
 // (8 chains) next to sub-partitions with one.  Here every sub-partition gets 7 chains: one warp of
 // 4 chains x 8 lanes (13 partner iterations) and one warp of 3 chains x 10 lanes (10 iterations, lanes
-// 30, 31 idle), 28 chains per CTA of 8 warps.  Instantiated for 97 <= N <= 100 (13 x 8 and 10 x 10 slots).
-template <typename Real, bool TRACE>
+// 30, 31 idle), 28 chains per CTA of 8 warps.  NA, NB = partner iterations of the two kinds of warp
+// (8 NA and 10 NB slots >= N); instantiated for the shapes listed in kMixed.
+template <typename Real, int NA, int NB, bool TRACE>
 __global__ void __launch_bounds__(256, 1) k_sweep_mixed(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
@@ -426,11 +427,28 @@ __global__ void __launch_bounds__(256, 1) k_sweep_mixed(const PtDev d, const PtL
   const int warp = threadIdx.x >> 5;
   const int cta0 = blockIdx.x * 28;
   if (warp < 4)
-    sweep_warp<Real, 8, 13, TRACE>(d, base + (size_t)(warp * 4) * pl.sstride, pl.sstride, 104, cta0 + warp * 4, 0, t0,
+    sweep_warp<Real, 8, NA, TRACE>(d, base + (size_t)(warp * 4) * pl.sstride, pl.sstride, 8 * NA, cta0 + warp * 4, 0, t0,
                                    n_sweeps);
   else
-    sweep_warp<Real, 10, 10, TRACE>(d, base + (size_t)16 * pl.sstride + (size_t)((warp - 4) * 3) * pl.sstride2,
-                                    pl.sstride2, 100, cta0 + 16 + (warp - 4) * 3, pl.stagger, t0, n_sweeps);
+    sweep_warp<Real, 10, NB, TRACE>(d, base + (size_t)16 * pl.sstride + (size_t)((warp - 4) * 3) * pl.sstride2,
+                                    pl.sstride2, 10 * NB, cta0 + 16 + (warp - 4) * 3, pl.stagger, t0, n_sweeps);
+}
+
+struct MixedVariant {
+  int NA, NB;
+  PtSweepFn f64[2], f32[2];   // [0] timed, [1] with the decision trace
+};
+#define PT_MIXED(NA, NB)                                                                     \
+  { NA, NB, { k_sweep_mixed<double, NA, NB, false>, k_sweep_mixed<double, NA, NB, true> },   \
+    { k_sweep_mixed<float, NA, NB, false>, k_sweep_mixed<float, NA, NB, true> } }
+// N = 51..56 (the paper's N = 55) and N = 97..100 (the throughput batch)
+const MixedVariant kMixed[] = { PT_MIXED(7, 6), PT_MIXED(13, 10) };
+
+const MixedVariant* find_mixed(int N)
+{
+  for (const MixedVariant& v : kMixed)
+    if ((N + 7) / 8 == v.NA && (N + 9) / 10 == v.NB) return &v;
+  return nullptr;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -557,8 +575,9 @@ SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
   if (pl.kind == PT_K_MIXED) {
-    if (precision == PT_F32) return trace ? (SweepFn)k_sweep_mixed<float, true> : (SweepFn)k_sweep_mixed<float, false>;
-    return trace ? (SweepFn)k_sweep_mixed<double, true> : (SweepFn)k_sweep_mixed<double, false>;
+    for (const MixedVariant& v : kMixed)
+      if (v.NA == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
+    return nullptr;
   }
   for (const SweepVariant& v : kVariants)
     if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
@@ -597,16 +616,17 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   }
   PtLaunch pl{};
   pl.lanes = L;
-  if (lanes_requested == 0 && L == 8 && d.N >= 97 && d.N <= 100 && (long long)d.C > 4 * smsp && (long long)d.C <= 7 * smsp) {
+  const MixedVariant* mv = find_mixed(d.N);
+  if (lanes_requested == 0 && L == 8 && mv && (long long)d.C > 4 * smsp && (long long)d.C <= 7 * smsp) {
     // between 4 and 7 chains per sub-partition: 4 + 3 chains on every one (k_sweep_mixed)
     const int Q = 128 / real_bytes;
     pl.kind = PT_K_MIXED;
-    pl.ni = 13;
-    pl.Ns = 104;
-    int ss = 3 * 104;
+    pl.ni = mv->NA;
+    pl.Ns = 8 * mv->NA;
+    int ss = 3 * pl.Ns;
     while (ss % Q != 8 % Q) ++ss;
     pl.sstride = ss;
-    ss = 3 * 100;
+    ss = 3 * 10 * mv->NB;
     while (ss % Q != 10 % Q) ++ss;
     pl.sstride2 = ss;
     pl.threads = 256;

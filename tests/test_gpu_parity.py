@@ -87,6 +87,26 @@ def test_config5_sampled_ensembles_of_the_full_batch():
         compare(ge, gte, o, otr, N=wl.N, nbins=nbins, hist=hist, label=f"config5 ensemble {e}")
 
 
+def test_mixed_mapping_at_the_papers_chain_length():
+    """N = 55, 40 ensembles x 64 replicas = 2560 chains: between 4 and 7 chains per SM sub-partition, so
+    the planner maps 4 chains x 8 lanes + 3 chains x 10 lanes on every one (k_sweep_mixed<7, 6>).  Sampled
+    ensembles against the oracle; they cover both kinds of warp."""
+    N, M, E = 55, 64, 40
+    T = synth.temperature_ladder(M, 0.15, 3.0)
+    w = synth.move_halfwidths(T)
+    conf = synth.random_walk_conformations(E, M, N, seed=5564)
+    seeds = synth.seeds(3, E, rank=3)
+    hist = hist_range(N)
+    g, gtr = run_gpu(N, M, E, T, w, seeds, conf, 30, 10, nbins=64, hist=hist)
+    assert g["launch_info"]["chains_per_cta"] == 28 and g["launch_info"]["lanes"] == 8
+    assert energy_close(g["energies"], g["energies_full"]).all()
+    for e in (0, 17, 39):
+        o, otr = run_oracle(N, M, 1, T, w, seeds[e:e + 1], conf[e:e + 1], 30, 10, nbins=64, hist=hist, e_offset=e)
+        ge = {k: v[e:e + 1] for k, v in g.items() if isinstance(v, np.ndarray)}
+        gte = {k: v[e:e + 1] for k, v in gtr.items()}
+        compare(ge, gte, o, otr, N=N, nbins=64, hist=hist, label=f"mixed N=55 ensemble {e}")
+
+
 def test_config5_full_length_invariants():
     """Config 5 at full size and length (10^3 sweeps) as bench.py times it: properties that hold at
     any size -- E_run equals the oracle's Eq.-4 energy of the returned conformation for sampled
