@@ -159,7 +159,11 @@ template <typename Real> struct BondChain {
     }
   }
   // stage point P of NPTS
-  template <int P, int NPTS> __device__ __forceinline__ void run() { range<(P * NLEV) / NPTS, ((P + 1) * NLEV) / NPTS>(); }
+  // stage point P of NPTS; LEVG = levels handed out over the stage points (the rest runs after the pair groups)
+  template <int P, int NPTS, int LEVG> __device__ __forceinline__ void run()
+  {
+    range<(P * LEVG) / NPTS, ((P + 1) * LEVG) / NPTS>();
+  }
   __device__ __forceinline__ void run_all() { range<0, NLEV>(); }
 };
 
@@ -175,12 +179,12 @@ constexpr int kGroupPoints = 14;   // stage points per pair group
 // one integer select, the count of inside pairs one predicated add.  A and C are applied once per
 // step by the caller.  The new squared distance follows from the old one:
 // |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
-template <typename Real, int L, int BEGIN, int CNT, int PBASE, int NPTS>
+template <typename Real, int L, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
 __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real (&en)[4],
                                            Real (&eo)[4], int& cnt, BondChain<Real>& side)
 {
-#define PT_SIDE(n) side.template run<PBASE + (n), NPTS>()
+#define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
   Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
 #pragma unroll
   for (int u = 0; u < CNT; ++u) X.get(lig + (BEGIN + u) * L, bx[u], by[u], bz[u]);
@@ -250,7 +254,7 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
 
 // The whole partner loop of NI > 0 iterations in groups of four (the last group takes the rest):
 // returns this lane's share of Delta E_LJ.
-template <typename Real, int L, int NI>
+template <typename Real, int L, int NI, int LEVG>
 __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
                                             Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
                                             BondChain<Real>& side)
@@ -259,7 +263,7 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
   Real en[4] = {(Real)0, (Real)0, (Real)0, (Real)0}, eo[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
   int cnt = 0;
 #define PT_PG(B, C, PB, NP) \
-  pair_group<Real, L, B, C, PB, NP>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt, side)
+  pair_group<Real, L, B, C, PB, NP, LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt, side)
   if (NI <= 7) {
     PT_PG(0, (NI <= 7 ? NI : 1), 0, P);
   } else if (NI <= 11) {
@@ -290,6 +294,11 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
 {
   static_assert(L >= 8 && L <= 32, "lanes per chain");
   constexpr int G = 32 / L;
+  // Short partner loops have fewer stage points than the bond stream has levels: one level per point,
+  // the rest of the stream runs behind the reduction of the pair sums (latency-bound shapes).
+  constexpr int NPTS = (NI <= 0 ? 0 : (NI <= 7 ? 1 : (NI <= 11 ? 2 : 3))) * kGroupPoints;
+  constexpr bool TAIL = NI > 0 && (L & (L - 1)) == 0 && NPTS < BondChain<Real>::NLEV;
+  constexpr int LEVG = TAIL ? NPTS : BondChain<Real>::NLEV;
   // lanes beyond G L (L = 10: lanes 30, 31) are ghosts: they repeat the last real lane and nobody reads them
   const int lane = min((int)(threadIdx.x & 31), G * L - 1);
   const int g = lane / L, lig = lane % L;
@@ -350,7 +359,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
       bc.xo = xo; bc.yo = yo; bc.zo = zo; bc.xn = xn; bc.yn = yn; bc.zn = zn; bc.u = p.u;
       Real part;
       if (NI > 0) {
-        part = pair_groups<Real, L, (NI > 0 ? NI : 1)>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
+        part = pair_groups<Real, L, (NI > 0 ? NI : 1), LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
       } else {
         bc.run_all();
         Real en = (Real)0, eo = (Real)0;
@@ -360,14 +369,40 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
           pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
         part = fma(-lj.C, (Real)cnt, en - eo);
       }
-      part += bc.bond;
-      const Real lg = bc.lg;
-      const bool broke = bc.broke;
-      const bool bond_broken = (__ballot_sync(0xffffffffu, broke) & bond_lanes) != 0u;
-      const Real logu = __shfl_sync(0xffffffffu, lg, gbase + 4);
-
-      // A4: reduce; every lane of the group gets the same Delta E
-      const Real dE = group_sum<Real, L>(part, lig, gbase);
+      Real dE, logu;
+      bool bond_broken;
+      if (TAIL) {
+        // A4 in two parts: the pair sums are reduced while the bond stream finishes (its last levels ride
+        // on the shuffle latencies); the bond terms sit in lanes 0..3 of the group and need two levels
+        Real v = part;
+        constexpr int REM = BondChain<Real>::NLEV - LEVG;
+        constexpr int NSH = L == 32 ? 5 : (L == 16 ? 4 : 3);
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        bc.template range<LEVG, LEVG + REM / NSH>();
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        bc.template range<LEVG + REM / NSH, LEVG + 2 * REM / NSH>();
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        bc.template range<LEVG + 2 * REM / NSH, LEVG + 3 * REM / NSH>();
+        if (L >= 16) {
+          v += __shfl_xor_sync(0xffffffffu, v, 8);
+          bc.template range<LEVG + 3 * REM / NSH, LEVG + 4 * REM / NSH>();
+        }
+        if (L == 32) {
+          v += __shfl_xor_sync(0xffffffffu, v, 16);
+          bc.template range<LEVG + 4 * REM / NSH, LEVG + REM>();
+        }
+        Real b = bc.bond;
+        b += __shfl_xor_sync(0xffffffffu, b, 1);
+        b += __shfl_xor_sync(0xffffffffu, b, 2);
+        bond_broken = (__ballot_sync(0xffffffffu, bc.broke) & bond_lanes) != 0u;
+        logu = __shfl_sync(0xffffffffu, bc.lg, gbase + 4);
+        dE = v + __shfl_sync(0xffffffffu, b, gbase);
+      } else {
+        bond_broken = (__ballot_sync(0xffffffffu, bc.broke) & bond_lanes) != 0u;
+        logu = __shfl_sync(0xffffffffu, bc.lg, gbase + 4);
+        // A4: reduce; every lane of the group gets the same Delta E
+        dE = group_sum<Real, L>(part + bc.bond, lig, gbase);
+      }
 
       // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
       const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
