@@ -8,7 +8,11 @@
 //        sqrt/log, the Metropolis exp) is one instruction stream shared by 32/L chains.
 // The paper's kernel (Listing 2) maps one replica to one block of 64 threads and
 // recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
-// long chains, and with the local Delta-E of Eq. (5) instead of the full sum.
+// very long chains (N > 480), and with the local Delta-E of Eq. (5) instead of the full sum.
+//
+// Kernels: k_sweep_group (L = 8, 16, 32 lanes per chain, partner loop unrolled in stage-major groups
+// with the bond stream interleaved), k_sweep_mixed (8- and 10-lane warps side by side against wave
+// quantisation), k_sweep_cta.  pt_plan_sweep chooses; DESIGN.md section 7 has the measurements.
 #include <math.h>
 
 #include "pt_sweep_common.cuh"

@@ -1,4 +1,4 @@
-// Pieces shared by the sweep kernels (pt_sweep.cu, pt_sweep_spec.cu): per-chain context, proposal,
+// Pieces shared by the sweep kernels of pt_sweep.cu: per-chain context, proposal,
 // once-per-sweep measurement.  Everything is static to its translation unit.
 #pragma once
 #include <math.h>
