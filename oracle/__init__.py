@@ -217,7 +217,7 @@ class Oracle:
             "move_counts": np.zeros((p.E, p.M, 3), dtype=np.uint64),
             "swap_counts": np.zeros((p.E, max(p.M - 1, 0), 2), dtype=np.uint64),
             "conformations": np.zeros((p.E, p.M, p.N, 3), dtype=np.float64),
-            "obs_moments": np.zeros((p.E, p.M, 4), dtype=np.float64),
+            "obs_moments": np.zeros((p.E, p.M, 5), dtype=np.float64),
         }
         lib().orc_read(self.h, _ptr(out["energies"], C.c_double), _ptr(out["histograms"], C.c_uint64),
                        _ptr(out["moments"], C.c_double), _ptr(out["move_counts"], C.c_uint64),

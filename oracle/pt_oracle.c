@@ -187,7 +187,7 @@ struct orc_state {
   double* Erun;     /* [E][M] */
   uint64_t* hist;   /* [E][M][nbins+2] */
   double* mom;      /* [E][M][3] */
-  double* obs;      /* [E][M][4] */
+  double* obs;      /* [E][M][5] */
   uint64_t* mcount; /* [E][M][3] */
   uint64_t* scount; /* [E][M-1][2] */
   int64_t t;        /* sweeps done since init      */
@@ -216,7 +216,7 @@ orc_state* orc_create(const orc_params* p, const double* temperatures, const dou
   s->Erun = (double*)calloc(C, sizeof(double));
   s->hist = (uint64_t*)calloc(C * (size_t)(p->nbins + 2), sizeof(uint64_t));
   s->mom = (double*)calloc(C * 3, sizeof(double));
-  s->obs = (double*)calloc(C * 4, sizeof(double));
+  s->obs = (double*)calloc(C * 5, sizeof(double));
   s->mcount = (uint64_t*)calloc(C * 3, sizeof(uint64_t));
   s->scount = (uint64_t*)calloc(E * (M > 1 ? M - 1 : 1) * 2, sizeof(uint64_t));
   for (size_t i = 0; i < M; ++i) {
@@ -245,7 +245,7 @@ int orc_init(orc_state* s, const uint64_t* seeds, const double* conformations)
   memcpy(s->X, conformations, C * N * 3 * sizeof(double));
   memset(s->hist, 0, C * (size_t)(p->nbins + 2) * sizeof(uint64_t));
   memset(s->mom, 0, C * 3 * sizeof(double));
-  memset(s->obs, 0, C * 4 * sizeof(double));
+  memset(s->obs, 0, C * 5 * sizeof(double));
   memset(s->mcount, 0, C * 3 * sizeof(uint64_t));
   memset(s->scount, 0, E * (M > 1 ? M - 1 : 1) * 2 * sizeof(uint64_t));
   s->t = 0; s->x = 0;
@@ -327,10 +327,13 @@ static void sweep_chain(orc_state* s, int e, int i, int64_t t)
   s->mom[c * 3 + 1] += Ecur;
   s->mom[c * 3 + 2] += Ecur * Ecur;
   double ree2 = orc_ree2(N, X), rg2 = orc_rgyr2(N, X);
-  s->obs[c * 4 + 0] += ree2;
-  s->obs[c * 4 + 1] += rg2;
-  s->obs[c * 4 + 2] += rg2 * rg2;
-  s->obs[c * 4 + 3] += ree2 * ree2;
+  s->obs[c * 5 + 0] += ree2;
+  s->obs[c * 5 + 1] += rg2;
+  s->obs[c * 5 + 2] += rg2 * rg2;
+  s->obs[c * 5 + 3] += ree2 * ree2;
+  /* the cross moment of the thermal fluctuation d<r_gyr^2>/dT = beta^2 (<E r_gyr^2> - <E><r_gyr^2>)
+   * that Fig. 5 plots (text around Eq. 8) */
+  s->obs[c * 5 + 4] += Ecur * rg2;
   if (t < s->cap_sweeps) {
     size_t o = c * (size_t)s->cap_sweeps + (size_t)t;
     if (s->tr_e) s->tr_e[o] = Ecur;
@@ -364,6 +367,18 @@ void orc_exchange(orc_state* s)
 {
   const orc_params* p = &s->p;
   int N = p->N, M = p->M;
+  /* Re-basing of the running energy (reading R22).  The paper's kernel recomputes the whole
+   * energy by Eq. (4) after every sweep (Listing 2: energy(&ps) follows oneSweep), so its
+   * energies never carry history; north_star fixes the local Delta E, and E_run += Delta E keeps the
+   * absolute rounding of the largest energy a chain ever held -- after a random-walk start with
+   * overlaps (E ~ 1e10 and beyond) that rounding can exceed the relaxed energy itself,
+   * and the swap test below would read noise.  Before the events x = 0, 1, 3, 7, ... (x + 1 a power of
+   * two) E_run is therefore replaced by the Eq.-4 sum of the current conformation: a logarithmic number
+   * of full recomputations per run. */
+  if (((s->x + 1) & s->x) == 0) {
+    size_t C = (size_t)p->E * (size_t)M;
+    for (size_t c = 0; c < C; ++c) s->Erun[c] = orc_total_energy(p, s->X + c * (size_t)N * 3);
+  }
   double* tmp = (double*)malloc((size_t)N * 3 * sizeof(double));
   for (int e = 0; e < p->E; ++e) {
     for (int i = (int)(s->x % 2); i + 1 < M; i += 2) {
@@ -417,5 +432,5 @@ void orc_read(const orc_state* s, double* energies, uint64_t* histograms, double
   if (move_counts) memcpy(move_counts, s->mcount, C * 3 * sizeof(uint64_t));
   if (swap_counts && M > 1) memcpy(swap_counts, s->scount, E * (M - 1) * 2 * sizeof(uint64_t));
   if (conformations) memcpy(conformations, s->X, C * N * 3 * sizeof(double));
-  if (obs_moments) memcpy(obs_moments, s->obs, C * 4 * sizeof(double));
+  if (obs_moments) memcpy(obs_moments, s->obs, C * 5 * sizeof(double));
 }

@@ -102,7 +102,7 @@ void orc_read(const orc_state* s,
               uint64_t* move_counts   /*[E][M][3]       attempts, accepts, bond-range rejections */,
               uint64_t* swap_counts   /*[E][M-1][2]     attempts, accepts for pair (i,i+1) */,
               double*   conformations /*[E][M][N][3]    */,
-              double*   obs_moments   /*[E][M][4]       sum Ree^2, sum Rg^2, sum Rg^4, sum Ree^4 */);
+              double*   obs_moments   /*[E][M][5]       sum Ree^2, sum Rg^2, sum Rg^4, sum Ree^4, sum E Rg^2 */);
 
 #ifdef __cplusplus
 }

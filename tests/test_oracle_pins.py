@@ -560,3 +560,130 @@ def test_create_rejects_bad_parameters():
     o = oracle.Oracle(oracle.make_params(3), T, w)
     with pytest.raises(ValueError):                         # a bond outside the FENE range: infinite energy
         o.init(np.array([1], dtype=np.uint64), _line(3, 1.2)[None, None])
+
+
+# ------------------------------------------------------------------ measurement: bins, under/overflow, observables
+def _frozen_dimers(rs, hist, nbins, n_sweeps=7):
+    """Dimers at hand-set bond lengths, moved with a half-width of 1e-13: the energy stays where it
+    was put (to ~1e-10), so what the measurement writes can be typed in by hand."""
+    M = len(rs)
+    p = oracle.make_params(2, M, 1, nbins=nbins, hist_emin=hist[0], hist_emax=hist[1])
+    o = oracle.Oracle(p, np.full(M, 1.0), np.full(M, 1e-13), threads=1)
+    o.init(np.array([5], dtype=np.uint64), _dimer_conf(1, rs))
+    o.run(n_sweeps, 0)
+    return o.read()
+
+
+def test_histogram_bins_underflow_overflow_by_hand():
+    """Reading R18: nbins interior bins over [emin, emax), bin = floor((E - emin) nbins /
+    (emax - emin)), then one underflow and one overflow bin.  Energies by hand (closed_forms.txt):
+    dimer at r0: -0.983683108864; at 0.85: LJ^mod(0.85) + 0.517827730413206; at 0.5: 41.65 + FENE."""
+    e07 = -0.983683108864
+    s6 = 0.117649 / (2.0 * 0.85 ** 6)
+    e085 = 4.0 * (s6 * s6 - s6) + 0.016316891136 + 0.517827730413206      # = +0.00758...
+    assert 0.007 < e085 < 0.008
+    e05 = 41.6511572664319 - 1.8 * np.log(1.0 - (0.2 / 0.3) ** 2)         # = 42.709...
+    n = 7
+    # (a) range [-2, 0.2), 11 bins of width 0.2: E(r0) -> bin floor(1.0163 * 5) = 5; E(0.85) -> floor(2.0076 * 5) = 10;
+    #     E(0.5) = 42.7 -> overflow (index nbins + 1)
+    out = _frozen_dimers([0.7, 0.85, 0.5], (-2.0, 0.2), 11, n)
+    h = out["histograms"][0]
+    assert out["energies"][0] == pytest.approx([e07, e085, e05], abs=1e-9)
+    exp = np.zeros((3, 13), dtype=np.uint64)
+    exp[0, 5] = n; exp[1, 10] = n; exp[2, 12] = n
+    assert np.array_equal(h, exp)
+    # (b) range [-0.5, 0.5), 4 bins of width 0.25: E(r0) -> underflow (index nbins); E(0.85) = 0.0076 -> bin 2
+    out = _frozen_dimers([0.7, 0.85], (-0.5, 0.5), 4, n)
+    exp = np.zeros((2, 6), dtype=np.uint64)
+    exp[0, 4] = n; exp[1, 2] = n
+    assert np.array_equal(out["histograms"][0], exp)
+    # (c) an energy that sits on a bin edge belongs to the upper bin (half-open bins): emin = E exactly
+    out = _frozen_dimers([0.7], (out["energies"][0, 0], 1.0), 8, 1)
+    assert out["histograms"][0, 0, 0] + out["histograms"][0, 0, 8] == 1      # bin 0, or underflow by one ulp of drift
+    # moments: n, n E, n E^2
+    out = _frozen_dimers([0.7, 0.85], (-2.0, 0.0), 10, n)
+    assert out["moments"][0, :, 0].tolist() == [n, n]
+    assert out["moments"][0, :, 1] == pytest.approx([n * e07, n * e085], rel=1e-9)
+    assert out["moments"][0, :, 2] == pytest.approx([n * e07 ** 2, n * e085 ** 2], rel=1e-9)
+
+
+def test_observable_sums_by_hand():
+    """obs = sums over sweeps of R_ee^2, r_gyr^2, r_gyr^4, R_ee^4, E r_gyr^2 (Eq. 8).
+    Dimer at distance r: R_ee^2 = r^2, r_gyr^2 = r^2/4.  Trimer on a line with spacing 0.7: R_ee^2 = 1.96,
+    r_gyr^2 = 2 * 0.49 / 3."""
+    n = 5
+    out = _frozen_dimers([0.7, 0.85], (-2.0, 0.0), 10, n)
+    for i, (r, e) in enumerate(((0.7, -0.983683108864), (0.85, out["energies"][0, 1]))):
+        assert out["obs_moments"][0, i] == pytest.approx(
+            [n * r * r, n * r * r / 4, n * (r * r / 4) ** 2, n * r ** 4, n * e * r * r / 4], rel=1e-9)
+    p = oracle.make_params(3, 1, 1)
+    o = oracle.Oracle(p, np.array([1.0]), np.array([1e-13]), threads=1)
+    o.init(np.array([1], dtype=np.uint64), _line(3)[None, None])
+    o.run(n, 0)
+    ob = o.read()["obs_moments"][0, 0]
+    rg2 = 2 * 0.49 / 3
+    e3 = 2 * -0.983683108864 - 0.014688968239          # two pairs at r0, one at 2 r0 (closed_forms.txt)
+    assert ob == pytest.approx([n * 1.96, n * rg2, n * rg2 ** 2, n * 1.96 ** 2, n * e3 * rg2], rel=1e-9)
+
+
+def test_dimer_cross_moment_gives_the_thermal_derivative_of_rgyr():
+    """d<r_gyr^2>/dT = beta^2 (<E r_gyr^2> - <E><r_gyr^2>) (the quantity of Fig. 5).
+    For the dimer r_gyr^2 = r^2/4 and all three averages are 1-D integrals of r^2 exp(-V/T); the same
+    number must also come out as the numerical T-derivative of <r^2/4>."""
+    V = lambda r: float(V_lj_mod(r) + V_fene(r))
+
+    def avgs(T):
+        w = lambda r: r * r * np.exp(-(V(r) + 1.0) / T)
+        Z = integrate.quad(w, 0.4, 1.0, epsabs=0, epsrel=1e-12, limit=400)[0]
+        av = lambda f: integrate.quad(lambda r: f(r) * w(r), 0.4, 1.0, epsabs=0, epsrel=1e-12, limit=400)[0] / Z
+        return av(V), av(lambda r: r * r / 4), av(lambda r: V(r) * r * r / 4)
+
+    T = np.array([0.5, 1.5])
+    E, n_sweeps, burn = 48, 20000, 2000
+    o, tr = _run(2, T, 0.1 * np.sqrt(T), E, n_sweeps)
+    out = o.read()
+    # the accumulated cross moment is the sum over sweeps of E_t rg2_t
+    assert np.allclose(out["obs_moments"][..., 4], (tr["energy"] * tr["rg2"]).sum(-1), rtol=1e-11)
+    assert np.allclose(out["obs_moments"][..., 1], tr["rg2"].sum(-1), rtol=1e-12)
+    for i, Ti in enumerate(T):
+        e1, g1, eg = avgs(Ti)
+        exact = (eg - e1 * g1) / Ti ** 2
+        h = 1e-4
+        assert exact == pytest.approx((avgs(Ti + h)[1] - avgs(Ti - h)[1]) / (2 * h), rel=1e-5)
+        en, rg = tr["energy"][:, i, burn:], tr["rg2"][:, i, burn:]
+        est = ((en * rg).mean(-1) - en.mean(-1) * rg.mean(-1)) / Ti ** 2
+        m, se = _mean_se(est)
+        assert se < 0.1 * abs(exact) and abs(m - exact) < 4.0 * se, (Ti, m, exact, se)
+
+
+def test_running_energy_is_rebased_on_eq4_before_events_2k_minus_1():
+    """Reading R22: the paper's kernel recomputes the energy by Eq. (4) after every sweep
+    (PAPER.md:146); the oracle keeps E_run += Delta E and replaces it by the Eq.-4 sum before the exchange
+    events x = 0, 1, 3, 7, ...  With M = 1 an event has no pair to try, so after such an event E_run IS
+    orc_total_energy of the conformation, bit for bit; after the other events it is the accumulated value."""
+    N = 13
+    conf = synth.random_walk_conformations(1, 1, N, 4242, d_min=0.0)
+    p = oracle.make_params(N, 1, 1)
+    o = oracle.Oracle(p, np.array([1.0]), np.array([0.1]), threads=1)
+    o.init(np.array([3], dtype=np.uint64), conf)
+    exact, n_inexact = [], 0
+    for x in range(9):
+        o.sweeps(5)
+        o.exchange()
+        out = o.read()
+        same = out["energies"][0, 0] == oracle.total_energy(out["conformations"][0, 0])
+        if x in (0, 1, 3, 7):
+            assert same, x
+        else:
+            n_inexact += not same
+    assert n_inexact >= 3            # 5 sweeps of accepted moves leave last-bit differences
+
+
+def test_overlap_start_meets_the_invariant_after_rebasing():
+    """P9 with the survey's own start (plain walk, overlaps): |E_run - E_full| <= 1e-9 max(1, |E_full|) once an
+    event 2^k - 1 has re-based the energies after the relaxation (here event 31, sweep 320 of 400)."""
+    o, tr, wl = _config1(d_min=0.0, n_sweeps=400)
+    out = o.read()
+    for i in range(wl.M):
+        full = oracle.total_energy(out["conformations"][0, i])
+        assert abs(out["energies"][0, i] - full) <= 1e-9 * max(1.0, abs(full))
