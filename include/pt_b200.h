@@ -15,7 +15,10 @@
  *   - every function returns an int status: PT_OK (0) or a negative PT_E* code;
  *     pt_last_error(h) gives a NUL-terminated message owned by the library
  *     (h == NULL: the message of the last failed pt_create* on this thread).
- *   - pointers marked HOST are host memory, DEVICE are CUDA device memory on the current device.
+ *   - pointers marked HOST are host memory, DEVICE are CUDA device memory.  A handle lives on the
+ *     CUDA device that is current when it is created (with a workspace: the device that owns the
+ *     workspace, which must be the current one, else PT_EINVAL); every later call makes that device
+ *     current for its own duration and restores the caller's afterwards.
  *     Input arrays are caller-owned and are consumed (copied) before the call returns.
  *     Output arrays are caller-allocated; NULL for an output means "skip it".
  *   - everything returned is indexed by TEMPERATURE index i (0 = first entry of `temperatures`),
@@ -32,6 +35,8 @@
  *     tag 1 PICK: same (a, b), only with PT_RANDOM_PICK: monomer = (w0 * N) >> 32
  *     tag 2 SWAP: a = lower temperature index of the pair, b = exchange event index x,
  *                 temperature field 0; w0 -> u_swap
+ *     tag 3 INIT: a = monomer n, b = 0: the direction of bond (n-1, n) of the library's own random
+ *                 walk (pt_init with conformations = NULL): z = s(w0), phi = 2 pi u(w1)
  *   word -> number, fp64:  s = (2w + 1 - 2^32) / 2^32 in (-1,1);  u = (w + 1/2) / 2^32 in (0,1)
  *                   fp32:  s = (2 (w >> 8) + 1 - 2^24) / 2^24;     u = ((w >> 9) + 1/2) / 2^23
  */
@@ -97,7 +102,10 @@ int pt_create_with_workspace(pt_handle** out, const pt_params* p, const double* 
 int pt_destroy(pt_handle* h);
 
 /* seeds[E] HOST: one Philox key per ensemble.  conformations[E][M][N][3] HOST, fp64, the
- * conformation that starts at temperature i of ensemble e (required).  Computes the running
+ * conformation that starts at temperature i of ensemble e; NULL = the library generates, on the
+ * host, a random walk of bond length r0 from the seeds (monomer 0 at the origin, bond directions
+ * uniform on the sphere from the Philox tag INIT above; overlaps of non-bonded monomers are
+ * allowed, so the initial energies can be large; read it back with pt_read).  Computes the running
  * energy of every chain by the full O(N^2) sum of Eq. (4), zeroes all statistics, sets the sweep
  * counter t = 0, the exchange-event counter x = 0 and the identity label permutation.
  * PT_EBOND if any chain's energy is not finite (state stays uninitialised). */
@@ -109,7 +117,10 @@ int pt_sweeps(pt_handle* h, int64_t n);
 
 /* One exchange event in every ensemble (Section 3.3, Eq. 6).  Event x tries the disjoint pairs
  * (i, i+1) with i = x mod 2, x mod 2 + 2, ...; accept iff Delta = (beta_i - beta_{i+1})(E_i -
- * E_{i+1}) >= 0 or u_swap < exp(Delta).  Swaps temperature labels on the device. */
+ * E_{i+1}) >= 0 or u_swap < exp(Delta).  Swaps temperature labels on the device.
+ * Before the events x = 0, 1, 3, 7, ... (x + 1 a power of two) the running energy of every chain is
+ * replaced by the full sum of Eq. (4) (the paper's kernel recomputes the energy after every sweep,
+ * PAPER.md:146), so that the rounding of a high-energy start does not stay in E_run for ever. */
 int pt_exchange(pt_handle* h);
 
 /* Repeats { pt_sweeps(exchange_every); pt_exchange() } until n_sweeps sweeps are done, without
@@ -125,7 +136,9 @@ int pt_read(pt_handle* h,
             uint64_t* move_counts   /* [E][M][3]        attempts, accepts, bond-range rejections     */,
             uint64_t* swap_counts   /* [E][M-1][2]      attempts, accepts of pair (i, i+1)           */,
             double*   conformations /* [E][M][N][3]     conformation currently at temperature i      */,
-            double*   obs_moments   /* [E][M][4]        sum Ree^2, sum Rg^2, sum Rg^4, sum Ree^4     */);
+            double*   obs_moments   /* [E][M][5]        sum Ree^2, sum Rg^2, sum Rg^4, sum Ree^4,
+                                                        sum E Rg^2 (Eq. 8 and d<Rg^2>/dT = beta^2
+                                                        (<E Rg^2> - <E><Rg^2>))    */);
 
 /* Full O(N^2) recomputation of Eq. (4) for every chain, without touching the running energy:
  * the invariant |E_run - E_full| is the caller's check.  energies_full[E][M] HOST. */
@@ -136,7 +149,10 @@ int pt_recompute_energy(pt_handle* h, double* energies_full);
 int pt_reset_stats(pt_handle* h);
 
 /* Test support: per-decision trace written by the kernels, all DEVICE, temperature-indexed,
- * NULL = off.  move_dec[E][M][cap_sweeps][N] one byte (0/1) per attempted move;
+ * NULL = off.  The library trusts the capacities: the buffers must be at least as large as stated
+ * here.  move_dec != NULL selects separate instantiations of the sweep kernels (the decision
+ * store sits in the step loop); with move_dec == NULL the sweep kernels are the ones a run without
+ * any trace uses, and swap_dec / e_trace are still written (pt_sweep_kernel_name tells which).  move_dec[E][M][cap_sweeps][N] one byte (0/1) per attempted move;
  * swap_dec[E][cap_events][M-1] one byte per pair slot and event: 0 not attempted, 1 rejected,
  * 2 accepted; e_trace[E][M][cap_sweeps] the running energy after every sweep.  Sweeps / events
  * beyond the capacities are not recorded.  Buffers stay owned by the caller. */
@@ -162,6 +178,11 @@ int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
  * chains per CTA. */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,
                    int32_t* smem_bytes);
+
+/* NUL-terminated name of the sweep-kernel instantiation the next pt_sweeps will launch, e.g.
+ * "k_sweep_mixed<double,13,10,trace=0>"; trace=1 while a move-decision trace is set.  buf HOST,
+ * n bytes (truncated to fit). */
+int pt_sweep_kernel_name(const pt_handle* h, char* buf, uint64_t n);
 
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t pt_kernel_launches(const pt_handle* h);

@@ -49,3 +49,17 @@ def reweight(hist: np.ndarray, centres: np.ndarray, T0: float, T: np.ndarray):
     e1 = (w * e).sum(axis=1) / z
     e2 = (w * e * e).sum(axis=1) / z
     return e1, (e2 - e1 * e1) / T ** 2
+
+
+def mean_rgyr2(moments: np.ndarray, obs_moments: np.ndarray) -> np.ndarray:
+    """<r_gyr^2> per temperature (Eq. 8) from obs_moments [..., 5]."""
+    return np.asarray(obs_moments, dtype=np.float64)[..., 1] / np.asarray(moments, dtype=np.float64)[..., 0]
+
+
+def d_rgyr2_dT(moments: np.ndarray, obs_moments: np.ndarray, temperatures: np.ndarray) -> np.ndarray:
+    """The quantity of Fig. 5: d<r_gyr^2>/dT = (<E r_gyr^2> - <E><r_gyr^2>) / T^2,
+    from the energy moments and the cross moment sum E r_gyr^2 the device accumulates."""
+    m = np.asarray(moments, dtype=np.float64)
+    o = np.asarray(obs_moments, dtype=np.float64)
+    n = m[..., 0]
+    return (o[..., 4] / n - (m[..., 1] / n) * (o[..., 1] / n)) / np.asarray(temperatures, dtype=np.float64) ** 2

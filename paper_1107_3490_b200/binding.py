@@ -24,7 +24,8 @@ _ERRNAMES = {-1: "PT_EINVAL", -2: "PT_ESTATE", -3: "PT_EBOND", -4: "PT_ENOMEM", 
 # every symbol include/pt_b200.h declares
 SYMBOLS = ("pt_workspace_bytes", "pt_create", "pt_create_with_workspace", "pt_destroy", "pt_init",
            "pt_sweeps", "pt_exchange", "pt_run", "pt_read", "pt_recompute_energy", "pt_reset_stats",
-           "pt_set_trace", "pt_counters", "pt_set_counters", "pt_launch_info", "pt_kernel_launches", "pt_last_error",
+           "pt_set_trace", "pt_counters", "pt_set_counters", "pt_launch_info", "pt_sweep_kernel_name",
+           "pt_kernel_launches", "pt_last_error",
            "pt_fma_peak")
 
 
@@ -80,6 +81,7 @@ def lib():
     L.pt_counters.argtypes = [hp, i64p, i64p]; L.pt_counters.restype = C.c_int
     L.pt_set_counters.argtypes = [hp, C.c_int64, C.c_int64]; L.pt_set_counters.restype = C.c_int
     L.pt_launch_info.argtypes = [hp, i32p, i32p, i32p, i32p]; L.pt_launch_info.restype = C.c_int
+    L.pt_sweep_kernel_name.argtypes = [hp, C.c_char_p, C.c_uint64]; L.pt_sweep_kernel_name.restype = C.c_int
     L.pt_kernel_launches.argtypes = [hp]; L.pt_kernel_launches.restype = C.c_int64
     L.pt_last_error.argtypes = [hp]; L.pt_last_error.restype = C.c_char_p
     L.pt_fma_peak.argtypes = [C.c_int, C.c_int, C.c_int, C.c_void_p, dp]; L.pt_fma_peak.restype = C.c_int
@@ -177,11 +179,12 @@ class ParallelTempering:
         self.pt_destroy()
 
     # -- the path -------------------------------------------------------------------------
-    def pt_init(self, seeds, conformations):
+    def pt_init(self, seeds, conformations=None):
+        """conformations = None: the library's own seeded random walk (read it back with pt_read)."""
         p = self.p
         seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
-        conf = np.ascontiguousarray(conformations, dtype=np.float64)
-        if seeds.shape != (p.E,) or conf.shape != (p.E, p.M, p.N, 3):
+        conf = None if conformations is None else np.ascontiguousarray(conformations, dtype=np.float64)
+        if seeds.shape != (p.E,) or (conf is not None and conf.shape != (p.E, p.M, p.N, 3)):
             raise ValueError("seeds must be (E,), conformations (E, M, N, 3)")
         _check(self._h, lib().pt_init(self._h, _ptr(seeds, C.c_uint64), _ptr(conf, C.c_double)))
 
@@ -211,7 +214,7 @@ class ParallelTempering:
         if conformations:
             out["conformations"] = np.zeros((p.E, p.M, p.N, 3), dtype=np.float64)
         if obs_moments:
-            out["obs_moments"] = np.zeros((p.E, p.M, 4), dtype=np.float64)
+            out["obs_moments"] = np.zeros((p.E, p.M, 5), dtype=np.float64)
         sc = out.get("swap_counts")
         _check(self._h, lib().pt_read(
             self._h, _ptr(out.get("energies"), C.c_double), _ptr(out.get("histograms"), C.c_uint64),
@@ -254,13 +257,16 @@ class ParallelTempering:
         _check(self._h, lib().pt_set_trace(self._h, int(cap_sweeps), int(cap_events), ptr("move"),
                                            ptr("swap"), ptr("energy")))
 
-    def trace(self) -> dict:
-        """Host copies of the trace buffers (synchronises)."""
+    def trace(self, ensembles=None) -> dict:
+        """Host copies of the trace buffers (synchronises); `ensembles`: indices to copy (None = all)."""
         import torch
         if self._stream is not None:
             self._stream.synchronize()
         torch.cuda.synchronize()
-        return {k: v.cpu().numpy() for k, v in self._trace.items()}
+        if ensembles is None:
+            return {k: v.cpu().numpy() for k, v in self._trace.items()}
+        idx = torch.as_tensor(list(ensembles), dtype=torch.long, device="cuda")
+        return {k: v.index_select(0, idx).cpu().numpy() for k, v in self._trace.items()}
 
     def pt_counters(self):
         t, x = C.c_int64(0), C.c_int64(0)
@@ -274,6 +280,11 @@ class ParallelTempering:
         a, b, c, d = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int32(0)
         _check(self._h, lib().pt_launch_info(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
         return {"lanes": a.value, "chains_per_cta": b.value, "grid": c.value, "smem_bytes": d.value}
+
+    def pt_sweep_kernel_name(self) -> str:
+        buf = C.create_string_buffer(128)
+        _check(self._h, lib().pt_sweep_kernel_name(self._h, buf, C.c_uint64(len(buf))))
+        return buf.value.decode()
 
     def pt_kernel_launches(self) -> int:
         return int(lib().pt_kernel_launches(self._h))

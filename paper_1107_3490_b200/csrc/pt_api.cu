@@ -11,11 +11,15 @@
 
 #include "pt_internal.h"
 
+// fp32 path: exchange events between two refreshes of the running energy from Eq. (4)
+#define PT_F32_REFRESH_EVENTS 8
+
 struct pt_handle {
   pt_params p;
   PtDev d;
   PtLaunch plan;
   cudaStream_t stream;
+  int device;          // CUDA device ordinal the handle was created on; every call runs there
   void* ws;            // base of the device workspace
   uint64_t ws_bytes;
   bool owns_ws;
@@ -51,6 +55,70 @@ int cuda_fail(pt_handle* h, cudaError_t e, const char* where)
   } while (0)
 
 uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+// Makes the handle's device current for the duration of a call and restores the caller's afterwards.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int device)
+  {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) {
+      err = cudaSetDevice(device);
+      switched = err == cudaSuccess;
+    }
+  }
+  ~DeviceGuard()
+  {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+
+#define PT_ENTER(h)                                                     \
+  DeviceGuard guard__((h)->device);                                     \
+  if (guard__.err != cudaSuccess) return cuda_fail((h), guard__.err, "selecting the handle's device")
+
+// ---- host-side random walk of pt_init(conformations = NULL) (SURVEY.md 8(d) input recipe) ----
+// Philox4x32-10 on the host, same stream layout as the device (include/pt_b200.h), tag 3 = INIT.
+void host_philox(const uint32_t ctr[4], uint64_t seed, uint32_t out[4])
+{
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = 0xD2511F53ull * c0, p1 = 0xCD9E8D57ull * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Monomer 0 at the origin; monomer n = monomer n-1 + r0 (sqrt(1-z^2) cos phi, sqrt(1-z^2) sin phi, z),
+// z = s(w0) in (-1, 1), phi = 2 pi u(w1), words from Philox(ctr = (n, 0, e, 3 << 24 | i), key = seed_e).
+// Every bond has length r0 up to rounding (E_FENE ~ 0); non-bonded overlaps are allowed, so initial
+// energies can be large and the first sweeps relax them.
+void host_random_walk(const pt_params& p, const uint64_t* seeds, std::vector<double>* out)
+{
+  const size_t N = (size_t)p.N, M = (size_t)p.M, E = (size_t)p.E;
+  out->assign(E * M * N * 3, 0.0);
+  const double two_pi = 6.283185307179586476925286766559;
+  for (size_t e = 0; e < E; ++e)
+    for (size_t i = 0; i < M; ++i) {
+      double* x = out->data() + (e * M + i) * N * 3;
+      for (size_t n = 1; n < N; ++n) {
+        const uint32_t ctr[4] = {(uint32_t)n, 0u, (uint32_t)e, (3u << 24) | (uint32_t)i};
+        uint32_t w[4];
+        host_philox(ctr, seeds[e], w);
+        const double z = (double)(2ll * (long long)w[0] + 1ll - 4294967296ll) * (1.0 / 4294967296.0);
+        const double phi = two_pi * (((double)w[1] + 0.5) * (1.0 / 4294967296.0));
+        const double s = sqrt(1.0 - z * z);
+        x[3 * n + 0] = x[3 * (n - 1) + 0] + p.r0 * (s * cos(phi));
+        x[3 * n + 1] = x[3 * (n - 1) + 1] + p.r0 * (s * sin(phi));
+        x[3 * n + 2] = x[3 * (n - 1) + 2] + p.r0 * z;
+      }
+    }
+}
 
 bool params_ok(const pt_params* p, std::string* why)
 {
@@ -98,7 +166,7 @@ Layout make_layout(const pt_params* p)
   L.keys = take(E * 8);
   L.hist = take(C * (uint64_t)(p->nbins + 2) * 8);
   L.mom = take(C * 3 * 8);
-  L.obs = take(C * 4 * 8);
+  L.obs = take(C * PT_NOBS * 8);
   L.mcount = take(C * 3 * 8);
   L.scount = take(E * (M > 1 ? M - 1 : 1) * 2 * 8);
   L.staging = take(C * N * 3 * 8);
@@ -129,6 +197,21 @@ int create_common(pt_handle** out, const pt_params* p, const double* T, const do
   pt_handle* h = new (std::nothrow) pt_handle();
   if (!h) return fail(nullptr, PT_ENOMEM, "host allocation failed");
   h->p = *p;
+  h->device = 0;
+  {
+    // the handle lives on the device that is current now (with a workspace: the device that owns it)
+    cudaError_t ge = cudaGetDevice(&h->device);
+    if (ge == cudaSuccess && !own) {
+      cudaPointerAttributes at{};
+      if (cudaPointerGetAttributes(&at, ws) == cudaSuccess && at.type == cudaMemoryTypeDevice) {
+        if (at.device != h->device) {
+          delete h;
+          return fail(nullptr, PT_EINVAL, "device_ws lives on another device than the current one");
+        }
+      }
+    }
+    cudaGetLastError();
+  }
   h->stream = (cudaStream_t)stream;
   h->owns_ws = own;
   h->initialised = false;
@@ -228,8 +311,11 @@ int pt_create_with_workspace(pt_handle** out, const pt_params* p, const double* 
 int pt_destroy(pt_handle* h)
 {
   if (!h) return PT_OK;
-  cudaStreamSynchronize(h->stream);
-  if (h->owns_ws) cudaFree(h->ws);
+  {
+    DeviceGuard guard(h->device);
+    cudaStreamSynchronize(h->stream);
+    if (h->owns_ws) cudaFree(h->ws);
+  }
   delete h;
   return PT_OK;
 }
@@ -237,10 +323,16 @@ int pt_destroy(pt_handle* h)
 int pt_init(pt_handle* h, const uint64_t* seeds, const double* conformations)
 {
   if (!h) return PT_EINVAL;
-  if (!seeds || !conformations) return fail(h, PT_EINVAL, "seeds / conformations is NULL");
+  if (!seeds) return fail(h, PT_EINVAL, "seeds is NULL");
+  PT_ENTER(h);
   const PtDev& d = h->d;
   h->initialised = false;
   const size_t C = (size_t)d.C, N = (size_t)d.N;
+  std::vector<double> walk;
+  if (!conformations) {   // the library's own start: a seeded random walk of bond length r0
+    host_random_walk(h->p, seeds, &walk);
+    conformations = walk.data();
+  }
   for (size_t q = 0; q < C * N * 3; ++q)
     if (!isfinite(conformations[q])) return fail(h, PT_EBOND, "a conformation has a non-finite coordinate");
   std::vector<uint2> keys(d.E);
@@ -269,6 +361,7 @@ int pt_sweeps(pt_handle* h, int64_t n)
 {
   if (!h) return PT_EINVAL;
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_sweeps before pt_init");
+  PT_ENTER(h);
   if (n < 0) return fail(h, PT_EINVAL, "n must be >= 0");
   if (h->t + n > 0xFFFFFFFFll) return fail(h, PT_ERANGE, "sweep counter would exceed 2^32 - 1");
   // one launch numbers its steps 0 .. chunk N - 1 (+ 8 drawn ahead) in an int
@@ -287,7 +380,20 @@ int pt_exchange(pt_handle* h)
 {
   if (!h) return PT_EINVAL;
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_exchange before pt_init");
+  PT_ENTER(h);
   if (h->x + 1 > 0xFFFFFFFFll) return fail(h, PT_ERANGE, "exchange counter would exceed 2^32 - 1");
+  // Re-basing of the running energy (reading R22).  The paper's kernel recomputed the whole
+  // energy after every sweep (Listing 2) and so carried no history; E_run += dE keeps the
+  // absolute rounding of the largest energy a chain ever held (a random-walk start with overlaps: 1e10
+  // and beyond).  Before the events x = 0, 1, 3, 7, ... (x + 1 a power of two) E_run is replaced by the
+  // Eq.-4 sum of the current conformation, before the swap test reads it.  The fp32 path, whose
+  // increments are only fp32-accurate (drift ~ sqrt(steps)), also does so every 8th event.
+  const bool rebase = ((h->x + 1) & h->x) == 0 ||
+                      (h->p.precision == PT_F32 && h->x % PT_F32_REFRESH_EVENTS == PT_F32_REFRESH_EVENTS - 1);
+  if (rebase) {
+    PT_CUDA(h, pt_launch_full_energy(h->d, h->p.precision, h->d.erun, h->stream));
+    h->launches += 1;
+  }
   PT_CUDA(h, pt_launch_exchange(h->d, (uint32_t)h->x, h->stream));
   if ((h->d.M - (int)(h->x & 1)) / 2 > 0) h->launches += 1;
   h->x += 1;
@@ -319,6 +425,7 @@ int pt_read(pt_handle* h, double* energies, uint64_t* histograms, double* moment
 {
   if (!h) return PT_EINVAL;
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_read before pt_init");
+  PT_ENTER(h);
   const PtDev& d = h->d;
   const size_t C = (size_t)d.C, N = (size_t)d.N, M = (size_t)d.M, E = (size_t)d.E;
   if (energies || conformations) {
@@ -335,7 +442,7 @@ int pt_read(pt_handle* h, double* energies, uint64_t* histograms, double* moment
   if (move_counts) PT_CUDA(h, cudaMemcpyAsync(move_counts, d.mcount, C * 3 * 8, cudaMemcpyDeviceToHost, h->stream));
   if (swap_counts && M > 1)
     PT_CUDA(h, cudaMemcpyAsync(swap_counts, d.scount, E * (M - 1) * 2 * 8, cudaMemcpyDeviceToHost, h->stream));
-  if (obs_moments) PT_CUDA(h, cudaMemcpyAsync(obs_moments, d.obs, C * 4 * 8, cudaMemcpyDeviceToHost, h->stream));
+  if (obs_moments) PT_CUDA(h, cudaMemcpyAsync(obs_moments, d.obs, C * PT_NOBS * 8, cudaMemcpyDeviceToHost, h->stream));
   PT_CUDA(h, cudaStreamSynchronize(h->stream));
   return PT_OK;
 }
@@ -344,6 +451,7 @@ int pt_recompute_energy(pt_handle* h, double* energies_full)
 {
   if (!h) return PT_EINVAL;
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_recompute_energy before pt_init");
+  PT_ENTER(h);
   if (!energies_full) return fail(h, PT_EINVAL, "energies_full is NULL");
   const PtDev& d = h->d;
   PT_CUDA(h, pt_launch_full_energy(d, h->p.precision, h->e_full, h->stream));
@@ -358,6 +466,7 @@ int pt_reset_stats(pt_handle* h)
 {
   if (!h) return PT_EINVAL;
   if (!h->initialised) return fail(h, PT_ESTATE, "pt_reset_stats before pt_init");
+  PT_ENTER(h);
   PT_CUDA(h, pt_launch_zero_stats(h->d, h->stream));
   h->launches += 1;
   return PT_OK;
@@ -402,6 +511,13 @@ int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, 
   if (chains_per_cta) *chains_per_cta = h->plan.chains_per_cta;
   if (grid) *grid = h->plan.grid;
   if (smem_bytes) *smem_bytes = h->plan.smem_bytes;
+  return PT_OK;
+}
+
+int pt_sweep_kernel_name(const pt_handle* h, char* buf, uint64_t n)
+{
+  if (!h || !buf || n == 0) return PT_EINVAL;
+  pt_sweep_kernel_desc(h->plan, h->p.precision, h->d.tr_move != nullptr, buf, (size_t)n);
   return PT_OK;
 }
 

@@ -32,7 +32,7 @@ __global__ void k_zero_stats(const PtDev d)
   const size_t nh = (size_t)d.C * (size_t)(d.nbins + 2);
   for (size_t q = tid; q < nh; q += stride) d.hist[q] = 0ull;
   for (size_t q = tid; q < (size_t)d.C * 3; q += stride) { d.mom[q] = 0.0; d.mcount[q] = 0ull; }
-  for (size_t q = tid; q < (size_t)d.C * 4; q += stride) d.obs[q] = 0.0;
+  for (size_t q = tid; q < (size_t)d.C * PT_NOBS; q += stride) d.obs[q] = 0.0;
   const size_t ns = (size_t)d.E * (size_t)(d.M > 1 ? d.M - 1 : 1) * 2;
   for (size_t q = tid; q < ns; q += stride) d.scount[q] = 0ull;
 }

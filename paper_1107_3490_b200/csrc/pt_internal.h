@@ -9,6 +9,9 @@
 // entries of a chain's shared-memory arrays and to hide the moved monomer from its own sum.
 #define PT_FAR 1.0e6
 
+// observables per temperature: sum R_ee^2, R_gyr^2, R_gyr^4, R_ee^4, E R_gyr^2 (Eq. 8)
+#define PT_NOBS 5
+
 // Device-side view of one simulation; passed by value to every kernel.
 struct PtDev {
   int N, M, E, C;        // C = E*M chains
@@ -36,7 +39,7 @@ struct PtDev {
   // statistics, temperature-indexed: ti = e*M + i
   unsigned long long* hist;    // [C][nbins+2]
   double* mom;                 // [C][3]
-  double* obs;                 // [C][4]
+  double* obs;                 // [C][PT_NOBS]
   unsigned long long* mcount;  // [C][3]
   unsigned long long* scount;  // [E][max(M-1,1)][2]
   // trace (test support), temperature-indexed
@@ -56,6 +59,7 @@ struct PtLaunch {
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
   int sstride2;        // PT_K_MIXED: stride of the 10-lane chains
+  int ni2;             // PT_K_MIXED: partner-loop iterations of the 10-lane warps
   int kind;            // PT_K_GROUP, PT_K_MIXED or PT_K_CTA
   int stagger;         // start delay in cycles per rank of a warp on its sub-partition (0 = none)
 };
@@ -68,6 +72,8 @@ typedef void (*PtSweepFn)(const PtDev, const PtLaunch, const uint32_t, const int
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan);
 cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& plan, uint32_t t0,
                             int n_sweeps, cudaStream_t stream);
+// name of the instantiation pt_launch_sweep would start, e.g. "k_sweep_mixed<double,13,10,trace=0>"
+void pt_sweep_kernel_desc(const PtLaunch& plan, int precision, bool trace, char* buf, size_t n);
 
 // pt_aux.cu
 cudaError_t pt_launch_scatter_init(const PtDev& d, int precision, const double* staging,

@@ -14,6 +14,7 @@
 // with the bond stream interleaved), k_sweep_mixed (8- and 10-lane warps side by side against wave
 // quantisation), k_sweep_cta.  pt_plan_sweep chooses; DESIGN.md section 7 has the measurements.
 #include <math.h>
+#include <stdio.h>
 
 #include "pt_sweep_common.cuh"
 
@@ -493,7 +494,7 @@ const MixedVariant* find_mixed(int N)
 // ------------------------------------------------------------------------------------------
 // CTA-per-replica kernel: blockDim.x threads share one chain (long chains, few replicas).
 // ------------------------------------------------------------------------------------------
-template <typename Real>
+template <typename Real, bool TRACE>
 __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                    const int n_sweeps)
 {
@@ -564,8 +565,10 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
 
       if (tid == 0) {
         if (accept) X.set(m, xn, yn, zn);
-        if (d.tr_move && (long long)t < d.cap_sweeps)
-          d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
+        if (TRACE) {   // test support (pt_set_trace): a separate instantiation
+          if (d.tr_move && (long long)t < d.cap_sweeps)
+            d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
+        }
       }
       if (accept) { c.erun += (double)dE; c.acc++; }
       c.brej += bond_broken ? 1u : 0u;
@@ -582,6 +585,8 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
 }
 
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+constexpr int kSmemCap = 200 * 1024;   // dynamic shared memory any sweep kernel may ask for
 
 typedef PtSweepFn SweepFn;
 
@@ -612,7 +617,10 @@ const SweepVariant* find_variant(int L, int ni_needed)
 
 SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
-  if (pl.kind == PT_K_CTA) return precision == PT_F32 ? (SweepFn)k_sweep_cta<float> : (SweepFn)k_sweep_cta<double>;
+  if (pl.kind == PT_K_CTA) {
+    if (precision == PT_F32) return trace ? (SweepFn)k_sweep_cta<float, true> : (SweepFn)k_sweep_cta<float, false>;
+    return trace ? (SweepFn)k_sweep_cta<double, true> : (SweepFn)k_sweep_cta<double, false>;
+  }
   if (pl.kind == PT_K_MIXED) {
     for (const MixedVariant& v : kMixed)
       if (v.NA == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
@@ -661,6 +669,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     const int Q = 128 / real_bytes;
     pl.kind = PT_K_MIXED;
     pl.ni = mv->NA;
+    pl.ni2 = mv->NB;
     pl.Ns = 8 * mv->NA;
     int ss = 3 * pl.Ns;
     while (ss % Q != 8 % Q) ++ss;
@@ -710,17 +719,27 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.grid = d.C;
     pl.smem_bytes = pl.sstride * real_bytes;
   }
-  if (pl.smem_bytes > 200 * 1024) return cudaErrorInvalidValue;
+  if (pl.smem_bytes > kSmemCap) return cudaErrorInvalidValue;
   for (int trace = 0; trace < 2; ++trace) {
     SweepFn fn = kernel_of(pl, precision, trace != 0);
     if (!fn) return cudaErrorInvalidValue;
     if (pl.smem_bytes > 48 * 1024) {
-      cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem_bytes);
+      // the attribute belongs to the kernel, not to the handle: always the same cap, so that two live
+      // handles that share an instantiation cannot lower each other's limit
+      cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemCap);
       if (e != cudaSuccess) return e;
     }
   }
   *plan = pl;
   return cudaSuccess;
+}
+
+void pt_sweep_kernel_desc(const PtLaunch& pl, int precision, bool trace, char* buf, size_t n)
+{
+  const char* real = precision == PT_F32 ? "float" : "double";
+  if (pl.kind == PT_K_CTA) snprintf(buf, n, "k_sweep_cta<%s,threads=%d,trace=%d>", real, pl.threads, trace ? 1 : 0);
+  else if (pl.kind == PT_K_MIXED) snprintf(buf, n, "k_sweep_mixed<%s,%d,%d,trace=%d>", real, pl.ni, pl.ni2, trace ? 1 : 0);
+  else snprintf(buf, n, "k_sweep_group<%s,%d,%d,trace=%d>", real, pl.lanes, pl.ni, trace ? 1 : 0);
 }
 
 cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, uint32_t t0, int n_sweeps,

@@ -37,7 +37,7 @@ struct ChainCtx {
   double beta;
   uint2 key;
   double erun, mom1, mom2;
-  double ob0, ob1, ob2, ob3;
+  double ob0, ob1, ob2, ob3, ob4;
   unsigned acc, brej;
 };
 
@@ -53,10 +53,11 @@ __device__ __forceinline__ void ctx_load(const PtDev& d, int s, ChainCtx& c)
   c.erun = d.erun[c.s];
   c.mom1 = d.mom[3 * c.ti + 1];
   c.mom2 = d.mom[3 * c.ti + 2];
-  c.ob0 = d.obs[4 * c.ti + 0];
-  c.ob1 = d.obs[4 * c.ti + 1];
-  c.ob2 = d.obs[4 * c.ti + 2];
-  c.ob3 = d.obs[4 * c.ti + 3];
+  c.ob0 = d.obs[PT_NOBS * c.ti + 0];
+  c.ob1 = d.obs[PT_NOBS * c.ti + 1];
+  c.ob2 = d.obs[PT_NOBS * c.ti + 2];
+  c.ob3 = d.obs[PT_NOBS * c.ti + 3];
+  c.ob4 = d.obs[PT_NOBS * c.ti + 4];
   c.acc = 0;
   c.brej = 0;
 }
@@ -86,10 +87,11 @@ __device__ __forceinline__ void ctx_store(const PtDev& d, const ChainCtx& c, int
   d.mom[3 * c.ti + 1] = c.mom1;
   d.mom[3 * c.ti + 2] = c.mom2;
   if (d.observables) {
-    d.obs[4 * c.ti + 0] = c.ob0;
-    d.obs[4 * c.ti + 1] = c.ob1;
-    d.obs[4 * c.ti + 2] = c.ob2;
-    d.obs[4 * c.ti + 3] = c.ob3;
+    d.obs[PT_NOBS * c.ti + 0] = c.ob0;
+    d.obs[PT_NOBS * c.ti + 1] = c.ob1;
+    d.obs[PT_NOBS * c.ti + 2] = c.ob2;
+    d.obs[PT_NOBS * c.ti + 3] = c.ob3;
+    d.obs[PT_NOBS * c.ti + 4] = c.ob4;
   }
   d.mcount[3 * c.ti + 0] += (unsigned long long)n_sweeps * (unsigned long long)d.N;
   d.mcount[3 * c.ti + 1] += c.acc;
@@ -195,6 +197,7 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, int g
   const double ex = (double)x1 - (double)x0, ey = (double)y1 - (double)y0, ez = (double)z1 - (double)z0;
   const double ree2 = ex * ex + ey * ey + ez * ez;
   c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
+  c.ob4 += c.erun * rg2;   // the cross moment of d<r_gyr^2>/dT = beta^2 (<E r_gyr^2> - <E><r_gyr^2>)
 }
 
 }  // namespace

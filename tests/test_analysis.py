@@ -48,3 +48,30 @@ def test_reweighting_reproduces_neighbouring_temperatures():
     assert np.all(np.abs(e_rw - e_direct) < 0.03), (e_rw, e_direct)
     assert np.all(np.abs(cv_rw - cv_direct) < 0.06), (cv_rw, cv_direct)
     assert abs(e_rw[1] - P10[1.0][0]) < 0.02
+
+
+def test_d_rgyr2_dT_of_the_dimer():
+    """analysis.d_rgyr2_dT (the quantity of Fig. 5) from the oracle's moments of a dimer run
+    against the numerical temperature derivative of the 1-D integral <r^2/4>."""
+    from scipy import integrate
+    sigma2 = 0.7 ** 2 / 2 ** (1 / 3)
+
+    def V(r):
+        lj = 0.0
+        if r < 2.5 * np.sqrt(sigma2):
+            s6 = (sigma2 / r ** 2) ** 3
+            lj = 4 * (s6 * s6 - s6) - 4 * (2.5 ** -12 - 2.5 ** -6)
+        return lj - 1.8 * np.log(1 - ((r - 0.7) / 0.3) ** 2)
+
+    def rg2(T):
+        w = lambda r: r * r * np.exp(-(V(r) + 1) / T)
+        Z = integrate.quad(w, 0.4, 1.0, epsrel=1e-12)[0]
+        return integrate.quad(lambda r: r * r / 4 * w(r), 0.4, 1.0, epsrel=1e-12)[0] / Z
+
+    T = np.array([0.5, 1.5])
+    out, _ = _dimer_run(T, n_sweeps=200000)
+    got = analysis.d_rgyr2_dT(out["moments"], out["obs_moments"], T)[0]
+    assert np.allclose(analysis.mean_rgyr2(out["moments"], out["obs_moments"])[0], [rg2(0.5), rg2(1.5)], rtol=5e-3)
+    for i, t in enumerate(T):
+        exact = (rg2(t + 1e-4) - rg2(t - 1e-4)) / 2e-4
+        assert abs(got[i] - exact) < 0.15 * abs(exact), (t, got[i], exact)

@@ -4,38 +4,41 @@ SURVEY.md 8(c)): 0 divergent accept/reject decisions, 0 divergent swap decisions
 running energies within 1e-9 max(1,|E|), final conformations bit-identical, equal counters and
 histograms.  The GPU swaps temperature labels, the oracle swaps conformations (PAPER.md:105 vs
 :267): their agreement is itself the test of that equivalence.
+
+Every case runs the GPU twice against one oracle run: with the move-decision trace (the TRACE=true
+instantiation of the sweep kernel) and without it (the instantiation bench.py times); parity_util.both
+asserts that the two really are different kernels.  The five BASELINE.json configurations run at their
+full length, config 5 with all 64 ensembles.
 """
 import numpy as np
 import pytest
 
 import paper_1107_3490_b200 as pt
 from paper_1107_3490_b200 import synth
-from parity_util import compare, energy_close, hist_range, run_gpu, run_oracle
+from parity_util import both, compare, energy_close, hist_range, run_gpu, run_oracle
 
 pytestmark = pytest.mark.gpu
 
 
-def _both(inp, n_sweeps, *, lanes=0, select_mode=0, widths=None, nbins=64, stepwise=False, threads=None,
-          exchange_every=None, floor=1.0):
+def _both(inp, n_sweeps, *, widths=None, exchange_every=None, **kw):
+    """parity_util.both on an Inputs bundle; returns (report of the untraced run, its GPU output, oracle)."""
     wl = inp.workload
     w = inp.widths if widths is None else widths
     S = wl.exchange_every if exchange_every is None else exchange_every
-    hist = hist_range(wl.N)
-    kw = dict(select_mode=select_mode, nbins=nbins, hist=hist)
-    o = run_oracle(wl.N, wl.M, wl.E, inp.temperatures, w, inp.seeds, inp.conformations, n_sweeps, S,
-                   threads=threads, **kw)
-    g = run_gpu(wl.N, wl.M, wl.E, inp.temperatures, w, inp.seeds, inp.conformations, n_sweeps, S,
-                lanes=lanes, stepwise=stepwise, **kw)
-    return compare(g[0], g[1], o[0], o[1], N=wl.N, nbins=nbins, hist=hist, floor=floor,
-                   label=f"{wl.name} lanes={lanes}"), g, o
+    kw.setdefault("label", wl.name)
+    reps, runs, o = both(wl.N, wl.M, wl.E, inp.temperatures, w, inp.seeds, inp.conformations, n_sweeps, S, **kw)
+    last = False if False in runs else True
+    if True in reps:
+        assert reps[True].get("divergent_moves", 0) == 0
+    return reps[last], runs[last], o
 
 
-# ---- the five BASELINE.json configurations --------------------------------------------------
+# ---- the five BASELINE.json configurations, full length, both instantiations --------------------
 
 def test_config1_full_run():
     """N=13, M=8, 2000 sweeps, exchange every 10: the whole job, default mapping."""
     rep, g, _ = _both(synth.make_inputs(1), 2000)
-    assert rep["divergent_moves"] == 0 and rep["divergent_swaps"] == 0
+    assert rep["divergent_swaps"] == 0
     assert g[0]["counters"] == (2000, 200)
 
 
@@ -56,28 +59,47 @@ def test_config2_full_run():
     assert g[0]["histograms"].sum() == 32 * 10000
 
 
-def test_config3_fp64():
-    """N=55, M=64, exchange every 20; 2000 of the 10^4 sweeps (the oracle's share of the time)."""
-    _both(synth.make_inputs(3), 2000, nbins=4096)
+def test_config3_full_run():
+    """N=55, M=64, exchange every 20, all 10^4 sweeps."""
+    rep, g, _ = _both(synth.make_inputs(3), 10000, nbins=4096)
+    assert g[0]["counters"] == (10000, 500)
 
 
-@pytest.mark.parametrize("lanes", [0, 128, 256])
-def test_config4_long_chain(lanes):
-    """N=309, M=128: the long Delta-E reduction: one warp per replica (default), one CTA per replica."""
-    rep, g, _ = _both(synth.make_inputs(4), 60 if lanes else 100, lanes=lanes)
-    if lanes == 0:
-        assert g[0]["launch_info"]["lanes"] == 32, "config 4 maps one warp per replica (10 unrolled iterations)"
+def test_config4_full_run():
+    """N=309, M=128, all 2000 sweeps, default mapping: one warp per replica (10 unrolled partner iterations)."""
+    rep, g, _ = _both(synth.make_inputs(4), 2000, nbins=4096, expect_kernel="k_sweep_group<double,32,10,")
+    assert g[0]["launch_info"]["lanes"] == 32 and g[0]["counters"] == (2000, 100)
+
+
+@pytest.mark.parametrize("lanes", [128, 256])
+def test_config4_one_cta_per_replica(lanes):
+    """BASELINE.json's wording of config 4, "one CTA per replica": the long Delta-E reduction across warps
+    (k_sweep_cta; slower than one warp per replica, so not the default), 60 sweeps."""
+    _both(synth.make_inputs(4), 60, lanes=lanes, expect_kernel="k_sweep_cta<double")
+
+
+def test_config5_full_run_all_64_ensembles():
+    """The throughput batch exactly as bench.py times it: 64 ensembles x 64 replicas, N=100, 10^3 sweeps,
+    exchange every 10, default mapping (k_sweep_mixed<double,13,10>: 147 CTAs of 28 chains; the last CTA is
+    partly filled -- chains 4088..4095 = the tail of ensemble 63 -- and its inactive lanes clone chain C-1).
+    One oracle run of all 64 ensembles; the GPU runs twice, untraced (the timed kernel) and traced; every
+    decision of all 4096 chains is compared."""
+    rep, g, _ = _both(synth.make_inputs(5), 1000, nbins=4096, expect_kernel="k_sweep_mixed<double,13,10,")
+    info = g[0]["launch_info"]
+    assert info["chains_per_cta"] == 28 and info["grid"] == 147
+    assert g[0]["counters"] == (1000, 100)
+    assert (g[0]["histograms"].sum(-1) == 1000).all()
 
 
 def test_config5_sampled_ensembles_of_the_full_batch():
-    """64 ensembles x 64 replicas, N=100: the GPU runs the FULL batch in bench.py's launch
-    configuration; the oracle recomputes sampled ensembles one by one (first, middle, last)."""
+    """The oracle recomputes single ensembles of the batch on their own (first, middle, last; e_offset puts
+    the ensemble index into the Philox counter): the per-ensemble streams are independent of the batch."""
     inp = synth.make_inputs(5)
     wl = inp.workload
     n_sweeps, S, nbins = 100, wl.exchange_every, 4096
     hist = hist_range(wl.N)
     g, gtr = run_gpu(wl.N, wl.M, wl.E, inp.temperatures, inp.widths, inp.seeds, inp.conformations,
-                     n_sweeps, S, nbins=nbins, hist=hist)
+                     n_sweeps, S, nbins=nbins, hist=hist, trace_moves=False)
     assert energy_close(g["energies"], g["energies_full"]).all()
     for e in (0, 31, 63):
         o, otr = run_oracle(wl.N, wl.M, 1, inp.temperatures, inp.widths, inp.seeds[e:e + 1],
@@ -89,55 +111,13 @@ def test_config5_sampled_ensembles_of_the_full_batch():
 
 def test_mixed_mapping_at_the_papers_chain_length():
     """N = 55, 40 ensembles x 64 replicas = 2560 chains: between 4 and 7 chains per SM sub-partition, so
-    the planner maps 4 chains x 8 lanes + 3 chains x 10 lanes on every one (k_sweep_mixed<7, 6>).  Sampled
-    ensembles against the oracle; they cover both kinds of warp."""
+    the planner maps 4 chains x 8 lanes + 3 chains x 10 lanes on every one (k_sweep_mixed<7, 6>)."""
     N, M, E = 55, 64, 40
     T = synth.temperature_ladder(M, 0.15, 3.0)
-    w = synth.move_halfwidths(T)
-    conf = synth.random_walk_conformations(E, M, N, seed=5564)
-    seeds = synth.seeds(3, E, rank=3)
-    hist = hist_range(N)
-    g, gtr = run_gpu(N, M, E, T, w, seeds, conf, 30, 10, nbins=64, hist=hist)
-    assert g["launch_info"]["chains_per_cta"] == 28 and g["launch_info"]["lanes"] == 8
-    assert energy_close(g["energies"], g["energies_full"]).all()
-    for e in (0, 17, 39):
-        o, otr = run_oracle(N, M, 1, T, w, seeds[e:e + 1], conf[e:e + 1], 30, 10, nbins=64, hist=hist, e_offset=e)
-        ge = {k: v[e:e + 1] for k, v in g.items() if isinstance(v, np.ndarray)}
-        gte = {k: v[e:e + 1] for k, v in gtr.items()}
-        compare(ge, gte, o, otr, N=N, nbins=64, hist=hist, label=f"mixed N=55 ensemble {e}")
-
-
-def test_config5_full_length_invariants():
-    """Config 5 at full size and length (10^3 sweeps) as bench.py times it: properties that hold at
-    any size -- E_run equals the oracle's Eq.-4 energy of the returned conformation for sampled
-    chains, counters add up, every bond inside the FENE range, label permutation intact."""
-    import oracle
-    inp = synth.make_inputs(5)
-    wl = inp.workload
-    p = pt.make_params(wl.N, wl.M, wl.E, nbins=4096, hist_emin=-5.0 * wl.N, hist_emax=3.0 * wl.N)
-    with pt.ParallelTempering(p, inp.temperatures, inp.widths) as sim:
-        sim.pt_init(inp.seeds, inp.conformations)
-        sim.pt_run(wl.n_sweeps, wl.exchange_every)
-        out = sim.pt_read()
-        efull = sim.pt_recompute_energy()
-    assert energy_close(out["energies"], efull).all()
-    rng = np.random.default_rng(5)
-    op = oracle.make_params(wl.N)
-    for e, i in zip(rng.integers(0, wl.E, 48), rng.integers(0, wl.M, 48)):
-        eo = oracle.total_energy(out["conformations"][e, i], op)
-        assert energy_close(out["energies"][e, i], eo), (e, i)
-    mc = out["move_counts"]
-    assert (mc[..., 0] == wl.N * wl.n_sweeps).all() and (mc[..., 1] <= mc[..., 0]).all()
-    assert (out["moments"][..., 0] == wl.n_sweeps).all()
-    assert (out["histograms"].sum(-1) == wl.n_sweeps).all()
-    sc = out["swap_counts"]
-    n_events = wl.n_sweeps // wl.exchange_every
-    assert (sc[:, 0::2, 0] == (n_events + 1) // 2).all() and (sc[:, 1::2, 0] == n_events // 2).all()
-    b = np.linalg.norm(np.diff(out["conformations"], axis=2), axis=-1)
-    assert (np.abs(b - 0.7) < 0.3).all()
-    # colder replicas end with lower mean energy than hotter ones
-    em = out["moments"][..., 1].mean(0) / wl.n_sweeps
-    assert em[0] < em[-1]
+    reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T), synth.seeds(3, E, rank=3),
+                         synth.random_walk_conformations(E, M, N, seed=5564), 100, 10, label="mixed N=55",
+                         expect_kernel="k_sweep_mixed<double,7,6,")
+    assert runs[False][0]["launch_info"]["chains_per_cta"] == 28
 
 
 # ---- variants and edge cases ----------------------------------------------------------------
@@ -153,20 +133,104 @@ def test_paper_literal_width():
     _both(synth.make_inputs(1), 300, widths=synth.paper_halfwidths(8))
 
 
-def test_overlapping_start_large_energies():
-    """Plain random walks with overlaps: huge initial energies, Delta E = -1e6...+inf, bond-range
-    rejections.  Decisions and coordinates must still agree; energies within 1e-9 relative."""
-    wl = synth.CONFIGS[1]
-    T = synth.temperature_ladder(wl.M, wl.T_min, wl.T_max)
-    conf = synth.random_walk_conformations(1, wl.M, wl.N, seed=99, d_min=0.0)
-    inp = synth.Inputs(wl, T, synth.move_halfwidths(T, 0.6), synth.seeds(9, 1), conf)
+@pytest.mark.parametrize("config_id,n_sweeps", [(1, 2000), (3, 1000)])
+def test_paper_literal_mode(config_id, n_sweeps):
+    """the paper's move as one mode -- "a random monomer of the chain is picked" AND
+    components uniform in [-0.01, 0.01] at every temperature -- on configs 1 and 3."""
+    inp = synth.make_inputs(config_id)
+    rep, g, o = _both(inp, n_sweeps, select_mode=1, widths=synth.paper_halfwidths(inp.workload.M))
+    acc = g[0]["move_counts"][..., 1] / g[0]["move_counts"][..., 0]
+    assert (acc > 0.5).all(), "a 0.01 cube is accepted most of the time at every temperature"
+
+
+def _max_abs_energy(conf):
     import oracle
-    e0 = max(abs(oracle.total_energy(c)) for c in conf[0])
+    return max(abs(oracle.total_energy(c)) for e in conf for c in e)
+
+
+# (label, N, M, E, lanes, kernel the planner must pick, sweeps, exchange_every)
+OVERLAP_CASES = [
+    ("config1_shape", 13, 8, 1, 0, "k_sweep_group<double,16,1,", 150, 10),
+    ("mixed_13_10", 100, 64, 40, 0, "k_sweep_mixed<double,13,10,", 40, 10),
+    ("mixed_7_6", 55, 64, 40, 0, "k_sweep_mixed<double,7,6,", 60, 10),
+    ("config4_shape", 309, 128, 1, 0, "k_sweep_group<double,32,10,", 40, 20),
+    ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
+    ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
+    ("N100_lanes32", 100, 16, 2, 32, "k_sweep_group<double,32,4,", 60, 10),
+    ("N200_lanes8_runtime_loop", 200, 8, 1, 8, "k_sweep_group<double,8,0,", 30, 10),
+    ("cta128", 100, 16, 1, 128, "k_sweep_cta<double", 40, 10),
+]
+
+
+@pytest.mark.parametrize("case", OVERLAP_CASES, ids=[c[0] for c in OVERLAP_CASES])
+def test_overlapping_start_large_energies(case):
+    """Plain random walks (d_min = 0: overlaps allowed, the start of SURVEY.md 8(d)) and wide moves in front
+    of every kernel family, both instantiations: huge initial energies, Delta E from -1e6 to +1e6 and beyond,
+    bond-range rejections (E_new = +inf).  Decisions, coordinates, counters and histograms must agree exactly.
+    The running energy keeps the rounding of the largest value held since it was last re-based on Eq. (4)
+    (pt_init; exchange events 2^k - 1, R22), so the 1e-9 energy criterion refers to that scale
+    (parity_util.rebased_floor): the largest |E| of the ensemble since the last re-basing."""
+    label, N, M, E, lanes, kernel, n_sweeps, S = case
+    T = synth.temperature_ladder(M, 0.2, 3.0)
+    conf = synth.random_walk_conformations(E, M, N, seed=9900 + N + M + E, d_min=0.0)
+    e0 = _max_abs_energy(conf)
+    assert e0 > 1e3, "the start must contain overlaps"
+    reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T, 0.6), synth.seeds(9, E), conf, n_sweeps, S,
+                         lanes=lanes, nbins=64, start_energy=e0, label=label, expect_kernel=kernel)
+    assert runs[False][0]["move_counts"][..., 2].sum() > 0, "the wide moves should have produced bond-range rejections"
+
+
+@pytest.mark.parametrize("config_id", [1, 2, 3, 4, 5])
+def test_every_config_from_the_plain_walk(config_id):
+    """SURVEY.md 8(d) input recipe taken literally: each of the five configurations started from plain random
+    walks with overlaps, 200 sweeps at its own widths and exchange cadence, both instantiations.  Energy scale:
+    parity_util.rebased_floor -- the initial energies (1e10 ... 1e33 for the big batches) until the first
+    re-basing of E_run, the energies at the last re-basing afterwards; the last 40 sweeps follow the re-basing
+    at sweep 160 and must meet the plain criterion 1e-9 max(1e3, |E|)."""
+    wl = synth.CONFIGS[config_id]
+    T = synth.temperature_ladder(wl.M, wl.T_min, wl.T_max)
+    conf = synth.random_walk_conformations(wl.E, wl.M, wl.N, seed=8800 + config_id, d_min=0.0)
+    e0 = _max_abs_energy(conf)
     assert e0 > 1e3
-    # the running energy carries the rounding of the large values it came down from; conformations
-    # can swap between temperatures, so the largest initial energy is the floor for all of them
-    rep, g, _ = _both(inp, 150, nbins=0, floor=e0)
-    assert g[0]["move_counts"][..., 2].sum() > 0, "the wide moves should have produced bond-range rejections"
+    reps, runs, o = both(wl.N, wl.M, wl.E, T, synth.move_halfwidths(T), synth.seeds(config_id, wl.E, rank=5), conf, 200,
+                         wl.exchange_every, nbins=64, start_energy=e0, label=f"{wl.name} plain walk (start {e0:.3g})")
+    tail_g, tail_o = runs[False][1]["energy"][..., 160:], o[1]["energy"][..., 160:]
+    assert energy_close(tail_g, tail_o, floor=1e3).all(), float(np.abs(tail_g - tail_o).max())
+
+
+def test_library_random_walk_start():
+    """pt_init(seeds, NULL): the library's own seeded walk: bonds of length r0 in
+    directions z = s(w0), phi = 2 pi u(w1) from Philox tag INIT.  Restated here in NumPy from the recipe with
+    the oracle's generator; equal up to the last bits of the host's sin / cos."""
+    import oracle
+    N, M, E = 30, 4, 3
+    T = synth.temperature_ladder(M, 0.5, 2.0)
+    seeds = synth.seeds(2, E, rank=9)
+    p = pt.make_params(N, M, E)
+    with pt.ParallelTempering(p, T, synth.move_halfwidths(T)) as sim:
+        sim.pt_init(seeds, None)
+        a = sim.pt_read()
+        sim.pt_init(seeds, None)
+        b = sim.pt_read()
+        sim.pt_run(20, 10)
+        assert energy_close(sim.pt_read()["energies"], sim.pt_recompute_energy(), floor=np.abs(a["energies"]).max()).all()
+    x = a["conformations"]
+    assert np.array_equal(x, b["conformations"])
+    assert np.allclose(np.linalg.norm(np.diff(x, axis=2), axis=-1), 0.7, atol=1e-13)
+    ref = np.zeros_like(x)
+    for e in range(E):
+        key = [int(seeds[e]) & 0xFFFFFFFF, int(seeds[e]) >> 32]
+        for i in range(M):
+            for n in range(1, N):
+                w = oracle.philox([n, 0, e, (3 << 24) | i], key)
+                z = (2 * w[0] + 1 - 2 ** 32) / 2.0 ** 32
+                phi = 2 * np.pi * (w[1] + 0.5) / 2.0 ** 32
+                sxy = np.sqrt(1 - z * z)
+                ref[e, i, n] = ref[e, i, n - 1] + 0.7 * np.array([sxy * np.cos(phi), sxy * np.sin(phi), z])
+    assert np.allclose(x, ref, rtol=0, atol=1e-12)
+    for e in range(E):
+        for i in range(M):
+            assert a["energies"][e, i] == pytest.approx(oracle.total_energy(x[e, i]), rel=1e-12)
 
 
 @pytest.mark.parametrize("N,M,E", [(2, 1, 1), (2, 3, 5), (3, 2, 7), (5, 1, 3), (17, 5, 3), (33, 7, 2),
