@@ -206,9 +206,10 @@ template <> struct PtNum<float> {
 // The sums accumulate u (A u - B) with u = 0 for the pairs outside the cutoff, and count the pairs
 // inside; the caller subtracts C * count once per sum.
 template <typename Real> struct PtLJ {
-  Real A, nB, C, rc2, c;   // c = B / A = sigma^-6
+  Real A, nB, C, rc2, c, mhc;   // c = B / A = sigma^-6, mhc = -c / 2
   __device__ __forceinline__ explicit PtLJ(const PtDev& d)
-      : A((Real)d.ljA), nB((Real)-d.ljB), C((Real)d.ljC), rc2((Real)d.rc2), c((Real)(d.ljB / d.ljA))
+      : A((Real)d.ljA), nB((Real)-d.ljB), C((Real)d.ljC), rc2((Real)d.rc2), c((Real)(d.ljB / d.ljA)),
+        mhc((Real)(-0.5 * (d.ljB / d.ljA)))
   {
   }
   // acc += u (A u - B) for one squared distance; returns whether it lies inside the cutoff
@@ -231,8 +232,8 @@ template <> struct PtVec2<float> { typedef float2 type; };
 template <typename Real> struct PtCoords {
   typename PtVec2<Real>::type* xy;
   Real* z;
-  __device__ __forceinline__ PtCoords(Real* base, int Ns)
-      : xy(reinterpret_cast<typename PtVec2<Real>::type*>(base)), z(base + 2 * (size_t)Ns)
+  __device__ __forceinline__ PtCoords(Real* base, int slots)
+      : xy(reinterpret_cast<typename PtVec2<Real>::type*>(base)), z(base + 2 * (size_t)slots)
   {
   }
   __device__ __forceinline__ void get(int j, Real& x, Real& y, Real& zz) const

@@ -177,22 +177,26 @@ constexpr int kGroupPoints = 14;   // stage points per pair group
 // A3 for CNT partner iterations at once (iterations BEGIN .. BEGIN+CNT-1 of this lane), written stage
 // by stage across the partners: every stage holds CNT or 2 CNT independent fp64 instructions, so that
 // a dependent instruction is not issued within the 8-cycle DFMA latency of its producer (written
-// partner by partner, ptxas kept one or two chains in flight).  Pairs inside the cutoff add
-// A u (u - c) - C with u = 1/r^6, c = B/A (Eq. 1-2); the others, and the moved monomer itself, get a
-// zero reciprocal seed, which stays zero through the Newton step and adds exactly nothing.  The
-// cutoff test is one DSETP (fp64 pipe) with the "not myself" mask as its predicate input, the mask
-// one integer select, the count of inside pairs one predicated add.  A and C are applied once per
-// step by the caller.  The new squared distance follows from the old one:
+// partner by partner, ptxas kept one or two chains in flight).
+//
+// Arithmetic (Eq. 1-2).  With u = 1/r^6 and c = B/A, E_LJ^mod = A u (u - c) - C inside the cutoff.
+// Per evaluation v = u - c/2 (one DFMA from x^2 and x = 1/r^2); per partner
+//   u_n (u_n - c) - u_o (u_o - c) = (v_n - v_o)(v_n + v_o):   DADD, DADD, DFMA.
+// A pair outside the cutoff, and the moved monomer itself, get a zero reciprocal seed (one FSEL), which stays
+// zero through the Newton step: u = 0, v = -c/2, and the partner adds exactly nothing unless it crosses the
+// cutoff.  The cutoff test is one DSETP (fp64 pipe) with the "not myself" mask as its predicate input, the
+// shift C needs the count of inside pairs (one predicated add); A and C are applied once per step by the
+// caller.  The new squared distance follows from the old one:
 // |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
-template <typename Real, int L, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
-__device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
-                                           Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd, Real (&en)[4],
-                                           Real (&eo)[4], int& cnt, BondChain<Real>& side)
+template <typename Real, int L, int NI, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
+__device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
+                                           Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
+                                           Real (&acc)[4], int& cnt, BondChain<Real>& side)
 {
 #define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
   Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) X.get(lig + (BEGIN + u) * L, bx[u], by[u], bz[u]);
+  for (int u = 0; u < CNT; ++u) X.get(s0 + (BEGIN + u) * L, bx[u], by[u], bz[u]);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) { bx[u] = xo - bx[u]; by[u] = yo - by[u]; bz[u] = zo - bz[u]; }
   PT_SIDE(0);
@@ -220,11 +224,11 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
   Real dv[2 * CNT], xv[2 * CNT], ev[2 * CNT];
 #pragma unroll
   for (int u = 0; u < CNT; ++u) {
-    const int j = lig + (BEGIN + u) * L;
+    const int j = s0 + (BEGIN + u) * L;
     dv[2 * u] = ro[u];
     dv[2 * u + 1] = rn[u];
-    xv[2 * u] = PtNum<Real>::template seed_if_inside<-1>(ro[u], lj.rc2, j, m, cnt);
-    xv[2 * u + 1] = PtNum<Real>::template seed_if_inside<1>(rn[u], lj.rc2, j, m, cnt);
+    xv[2 * u] = PtNum<Real>::template seed_if_inside<-1>(ro[u], lj.rc2, j, sm, cnt);
+    xv[2 * u + 1] = PtNum<Real>::template seed_if_inside<1>(rn[u], lj.rc2, j, sm, cnt);
   }
   PT_SIDE(8);
   if (PtNum<Real>::kNewton) {
@@ -244,44 +248,53 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
   for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] * xv[v];
   PT_SIDE(11);
 #pragma unroll
-  for (int v = 0; v < 2 * CNT; ++v) xv[v] = ev[v] * xv[v];          // u = 1/r^6
+  for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(ev[v], xv[v], lj.mhc);          // v = 1/r^6 - c/2
   PT_SIDE(12);
 #pragma unroll
-  for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] - lj.c;
+  for (int u = 0; u < CNT; ++u) {
+    ev[2 * u] = xv[2 * u + 1] - xv[2 * u];
+    ev[2 * u + 1] = xv[2 * u + 1] + xv[2 * u];
+  }
   PT_SIDE(13);
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) {
-    eo[(BEGIN + u) & 3] = fma(xv[2 * u], ev[2 * u], eo[(BEGIN + u) & 3]);
-    en[(BEGIN + u) & 3] = fma(xv[2 * u + 1], ev[2 * u + 1], en[(BEGIN + u) & 3]);
-  }
+  for (int u = 0; u < CNT; ++u) acc[(BEGIN + u) & 3] = fma(ev[2 * u], ev[2 * u + 1], acc[(BEGIN + u) & 3]);
 #undef PT_SIDE
 }
 
-// The whole partner loop of NI > 0 iterations in groups of four (the last group takes the rest):
-// returns this lane's share of Delta E_LJ.
+// How the NI partner iterations of a lane are cut into groups (each group is one stage-major block of
+// pair_group).  Balanced groups of at most kMaxGroup partners: 13 -> 5 + 4 + 4, 10 -> 5 + 5, <= 5 -> one group.
+// Measured on B200 (config 5): 5 + 4 + 4 / 5 + 5 is 3 % faster than 4 + 4 + 5 / 4 + 6.
+#ifndef PT_MAXGROUP
+#define PT_MAXGROUP 5
+#endif
+constexpr int kMaxGroup = PT_MAXGROUP;
+__host__ __device__ constexpr int n_groups(int NI) { return NI <= 0 ? 0 : (NI + kMaxGroup - 1) / kMaxGroup; }
+// size and first iteration of group g: the first (NI mod n) groups get one more
+__host__ __device__ constexpr int group_size(int NI, int g) { return NI / n_groups(NI) + (g < NI % n_groups(NI) ? 1 : 0); }
+__host__ __device__ constexpr int group_begin(int NI, int g) { return g == 0 ? 0 : group_begin(NI, g - 1) + group_size(NI, g - 1); }
+
+// The whole partner loop of NI > 0 iterations: returns this lane's share of Delta E_LJ.
+// s0 = this lane's first partner, sm = the moved monomer (its own slot is masked out).
 template <typename Real, int L, int NI, int LEVG>
-__device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int lig, int m, Real xo,
-                                            Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
+__device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
+                                            Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
                                             BondChain<Real>& side)
 {
   constexpr int P = kGroupPoints;
-  Real en[4] = {(Real)0, (Real)0, (Real)0, (Real)0}, eo[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
+  constexpr int NG = n_groups(NI);
+  static_assert(NG >= 1 && NG <= 4, "add a group");
+  Real acc[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
   int cnt = 0;
-#define PT_PG(B, C, PB, NP) \
-  pair_group<Real, L, B, C, PB, NP, LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt, side)
-  if (NI <= 7) {
-    PT_PG(0, (NI <= 7 ? NI : 1), 0, P);
-  } else if (NI <= 11) {
-    PT_PG(0, 4, 0, 2 * P);
-    PT_PG(4, (NI > 7 && NI <= 11 ? NI - 4 : 1), P, 2 * P);
-  } else {
-    static_assert(NI <= 15, "add a group");
-    PT_PG(0, 4, 0, 3 * P);
-    PT_PG(4, 4, P, 3 * P);
-    PT_PG(8, (NI > 11 ? NI - 8 : 1), 2 * P, 3 * P);
-  }
+#define PT_PG(g)                                                                                             \
+  if (NG > g)                                                                                                \
+    pair_group<Real, L, NI, group_begin(NI, g < NG ? g : 0), group_size(NI, g < NG ? g : 0), g * P, NG * P, LEVG>( \
+        lj, X, s0, sm, xo, yo, zo, tdx, tdy, tdz, dd, acc, cnt, side)
+  PT_PG(0);
+  PT_PG(1);
+  PT_PG(2);
+  PT_PG(3);
 #undef PT_PG
-  return fma(lj.A, ((en[0] - eo[0]) + (en[1] - eo[1])) + ((en[2] - eo[2]) + (en[3] - eo[3])), -lj.C * (Real)cnt);
+  return fma(lj.A, (acc[0] + acc[1]) + (acc[2] + acc[3]), -lj.C * (Real)cnt);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -301,7 +314,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
   constexpr int G = 32 / L;
   // Short partner loops have fewer stage points than the bond stream has levels: one level per point,
   // the rest of the stream runs behind the reduction of the pair sums (latency-bound shapes).
-  constexpr int NPTS = (NI <= 0 ? 0 : (NI <= 7 ? 1 : (NI <= 11 ? 2 : 3))) * kGroupPoints;
+  constexpr int NPTS = n_groups(NI) * kGroupPoints;
   constexpr bool TAIL = NI > 0 && (L & (L - 1)) == 0 && NPTS < BondChain<Real>::NLEV;
   constexpr int LEVG = TAIL ? NPTS : BondChain<Real>::NLEV;
   // lanes beyond G L (L = 10: lanes 30, 31) are ghosts: they repeat the last real lane and nobody reads them
@@ -412,7 +425,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
       // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
       const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
 
-      // A7: commit (branch-free: one predicated store pair, selects for the bookkeeping)
+      // A7: commit (branch-free: predicated stores, selects for the bookkeeping)
       if (accept && lig == 0) X.set(m, xn, yn, zn);
       if (TRACE) {   // test support (pt_set_trace): a separate instantiation, the timed one has no branch here
         if (lig == 0 && d.tr_move && c.active && (long long)t < d.cap_sweeps)
@@ -425,7 +438,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
     }
 
     // A8: measurement once per sweep
-    if (d.observables) measure_shape<Real, L>(c, N, lig, gbase, X);
+    if (d.observables) measure_shape<Real, L>(d, c, N, lig, gbase, X);
     if (leader) measure_energy(d, c, t);
   }
 
@@ -482,7 +495,11 @@ struct MixedVariant {
   { NA, NB, { k_sweep_mixed<double, NA, NB, false>, k_sweep_mixed<double, NA, NB, true> },   \
     { k_sweep_mixed<float, NA, NB, false>, k_sweep_mixed<float, NA, NB, true> } }
 // N = 51..56 (the paper's N = 55) and N = 97..100 (the throughput batch)
+#ifdef PT_FEW_VARIANTS
+const MixedVariant kMixed[] = { PT_MIXED(13, 10) };
+#else
 const MixedVariant kMixed[] = { PT_MIXED(7, 6), PT_MIXED(13, 10) };
+#endif
 
 const MixedVariant* find_mixed(int N)
 {
@@ -575,7 +592,7 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
       __syncthreads();
     }
 
-    if (d.observables && warp == 0) measure_shape<Real, 32>(c, N, lane, 0, X);
+    if (d.observables && warp == 0) measure_shape<Real, 32>(d, c, N, lane, 0, X);
     if (tid == 0) measure_energy(d, c, t);
   }
 
@@ -601,11 +618,16 @@ struct SweepVariant {
 // Unrolled instantiations (NI = partner-loop iterations); NI = 0 is the run-time loop of the same
 // lane count and must come last within its L.
 const SweepVariant kVariants[] = {
+#ifdef PT_FEW_VARIANTS
+    PT_VARIANT(8, 13), PT_VARIANT(8, 0), PT_VARIANT(16, 1), PT_VARIANT(16, 0), PT_VARIANT(32, 1), PT_VARIANT(32, 2),
+    PT_VARIANT(32, 10), PT_VARIANT(32, 0),
+#else
     PT_VARIANT(8, 2),  PT_VARIANT(8, 4),  PT_VARIANT(8, 7),  PT_VARIANT(8, 10), PT_VARIANT(8, 13),
     PT_VARIANT(8, 0),
     PT_VARIANT(16, 1), PT_VARIANT(16, 2), PT_VARIANT(16, 4), PT_VARIANT(16, 7), PT_VARIANT(16, 0),
     PT_VARIANT(32, 1), PT_VARIANT(32, 2), PT_VARIANT(32, 4), PT_VARIANT(32, 7), PT_VARIANT(32, 10),
     PT_VARIANT(32, 13), PT_VARIANT(32, 15), PT_VARIANT(32, 0),
+#endif
 };
 
 const SweepVariant* find_variant(int L, int ni_needed)

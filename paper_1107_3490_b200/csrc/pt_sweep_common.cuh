@@ -36,8 +36,8 @@ struct ChainCtx {
   bool active;
   double beta;
   uint2 key;
-  double erun, mom1, mom2;
-  double ob0, ob1, ob2, ob3, ob4;
+  double erun;
+  double mom1, mom2;
   unsigned acc, brej;
 };
 
@@ -53,16 +53,13 @@ __device__ __forceinline__ void ctx_load(const PtDev& d, int s, ChainCtx& c)
   c.erun = d.erun[c.s];
   c.mom1 = d.mom[3 * c.ti + 1];
   c.mom2 = d.mom[3 * c.ti + 2];
-  c.ob0 = d.obs[PT_NOBS * c.ti + 0];
-  c.ob1 = d.obs[PT_NOBS * c.ti + 1];
-  c.ob2 = d.obs[PT_NOBS * c.ti + 2];
-  c.ob3 = d.obs[PT_NOBS * c.ti + 3];
-  c.ob4 = d.obs[PT_NOBS * c.ti + 4];
   c.acc = 0;
   c.brej = 0;
 }
 
-// once per sweep, by one thread of the chain (A8): histogram, moments, energy trace
+// once per sweep, by one thread of the chain (A8): histogram, moments, energy trace.  A temperature index
+// is owned by exactly one chain during a launch, so no atomics are needed.  (The two energy sums stay in
+// registers: moving them to global memory changed ptxas' schedule of the step loop for the worse, +2 %.)
 __device__ __forceinline__ void measure_energy(const PtDev& d, ChainCtx& c, uint32_t t)
 {
   const double E = c.erun;
@@ -86,13 +83,6 @@ __device__ __forceinline__ void ctx_store(const PtDev& d, const ChainCtx& c, int
   d.mom[3 * c.ti + 0] += (double)n_sweeps;
   d.mom[3 * c.ti + 1] = c.mom1;
   d.mom[3 * c.ti + 2] = c.mom2;
-  if (d.observables) {
-    d.obs[PT_NOBS * c.ti + 0] = c.ob0;
-    d.obs[PT_NOBS * c.ti + 1] = c.ob1;
-    d.obs[PT_NOBS * c.ti + 2] = c.ob2;
-    d.obs[PT_NOBS * c.ti + 3] = c.ob3;
-    d.obs[PT_NOBS * c.ti + 4] = c.ob4;
-  }
   d.mcount[3 * c.ti + 0] += (unsigned long long)n_sweeps * (unsigned long long)d.N;
   d.mcount[3 * c.ti + 1] += c.acc;
   d.mcount[3 * c.ti + 2] += c.brej;
@@ -172,7 +162,8 @@ __device__ __forceinline__ Real bonds_and_logu(const PtDev& d, int role, int m, 
 
 // Eq. (8), and R_ee once per sweep; all lanes of the group take part.
 template <typename Real, int L>
-__device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, int gbase, const PtCoords<Real>& X)
+__device__ __forceinline__ void measure_shape(const PtDev& d, const ChainCtx& c, int N, int lig, int gbase,
+                                              const PtCoords<Real>& X)
 {
   double sx = 0.0, sy = 0.0, sz = 0.0;
   for (int j = lig; j < N; j += L) {
@@ -196,8 +187,11 @@ __device__ __forceinline__ void measure_shape(ChainCtx& c, int N, int lig, int g
   X.get(N - 1, x1, y1, z1);
   const double ex = (double)x1 - (double)x0, ey = (double)y1 - (double)y0, ez = (double)z1 - (double)z0;
   const double ree2 = ex * ex + ey * ey + ez * ez;
-  c.ob0 += ree2; c.ob1 += rg2; c.ob2 += rg2 * rg2; c.ob3 += ree2 * ree2;
-  c.ob4 += c.erun * rg2;   // the cross moment of d<r_gyr^2>/dT = beta^2 (<E r_gyr^2> - <E><r_gyr^2>)
+  if (lig == 0 && c.active) {
+    double* ob = d.obs + PT_NOBS * (size_t)c.ti;
+    ob[0] += ree2; ob[1] += rg2; ob[2] += rg2 * rg2; ob[3] += ree2 * ree2;
+    ob[4] += c.erun * rg2;   // the cross moment of d<r_gyr^2>/dT = beta^2 (<E r_gyr^2> - <E><r_gyr^2>)
+  }
 }
 
 }  // namespace
