@@ -17,11 +17,14 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libpt_b200.so"
-SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu"]
+OBJ = PKG / "build"
+# the sweep kernels are instantiated in several translation units so that they compile in parallel
+SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu", "pt_sweep_group.cu"] + \
+          [f"pt_sweep_comp{u}.cu" for u in range(8)]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-O3", "-std=c++17", "-lineinfo", "--threads", "0",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-O3", "-std=c++17", "-lineinfo",
+    "-Xcompiler", "-fPIC",
     "-I", str(ROOT / "include"), "-I", str(CSRC),
 ]
 
@@ -47,18 +50,35 @@ def is_stale() -> bool:
     return any(f.stat().st_mtime > t for f in _inputs())
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not is_stale():
-        return LIB
-    cmd = [_nvcc(), *NVCC_FLAGS]
+def _compile(nvcc: str, src: str, verbose: bool) -> Path:
+    obj = OBJ / (Path(src).stem + ".o")
+    cmd = [nvcc, *NVCC_FLAGS, "-c", "-o", str(obj), str(CSRC / src)]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    cmd += ["-o", str(LIB), *[str(CSRC / s) for s in SOURCES]]
     res = subprocess.run(cmd, cwd=str(CSRC), capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libpt_b200.so:\n" + res.stderr[-4000:])
+        raise RuntimeError(f"nvcc failed on {src}:\n" + res.stderr[-4000:])
+    return obj
+
+
+def build(force: bool = False, verbose: bool = False) -> Path:
+    """Compiles every translation unit (in parallel) and links libpt_b200.so."""
+    if not force and not is_stale():
+        return LIB
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    nvcc = _nvcc()
+    OBJ.mkdir(exist_ok=True)
+    workers = max(1, min(len(SOURCES), len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else 4))
+    with ThreadPoolExecutor(workers) as pool:
+        objs = list(pool.map(lambda s: _compile(nvcc, s, verbose), SOURCES))
+    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", str(LIB), *map(str, objs)]
+    res = subprocess.run(cmd, cwd=str(CSRC), capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed linking libpt_b200.so:\n" + res.stderr[-4000:])
     return LIB
 
 

@@ -49,6 +49,9 @@ struct PtDev {
   long long cap_sweeps, cap_events;
 };
 
+struct PtLaunch;
+typedef void (*PtSweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
+
 struct PtLaunch {
   int lanes;           // resolved lanes per chain
   int chains_per_cta;
@@ -58,15 +61,30 @@ struct PtLaunch {
   int sstride;         // shared-memory stride between chains, in Reals
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
-  int sstride2;        // PT_K_MIXED: stride of the 10-lane chains
-  int ni2;             // PT_K_MIXED: partner-loop iterations of the 10-lane warps
-  int kind;            // PT_K_GROUP, PT_K_MIXED or PT_K_CTA
-  int stagger;         // start delay in cycles per rank of a warp on its sub-partition (0 = none)
+  int kind;            // PT_K_GROUP, PT_K_COMP or PT_K_CTA
+  int stagger;         // PT_K_GROUP: start delay in cycles per rank of a warp on its sub-partition (0 = none)
+  // PT_K_COMP: warps of different kinds in one CTA (k_sweep_comp); kind 0, 1, 2, 3 = 8, 10, 16, 32 lanes per chain
+  int nik[4];          // partner-loop iterations of the four kinds of warp (template arguments of the kernel)
+  int kstride[4];      // shared-memory stride between the chains of a warp of each kind, in Reals
+  int wkind[8];        // kind of warp w
+  int wfirst[8];       // first chain of warp w within the CTA
+  int woff[8];         // shared-memory offset of warp w's first chain, in Reals
+  int wdelay[8];       // start delay of warp w in cycles
 };
 
-enum { PT_K_GROUP = 0, PT_K_MIXED = 1, PT_K_CTA = 2 };
+enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2 };
 
-typedef void (*PtSweepFn)(const PtDev, const PtLaunch, const uint32_t, const int);
+// Kernel tables, one per translation unit that instantiates sweep kernels (nullptr = not in this unit).
+PtSweepFn pt_lookup_group(int lanes, int ni, int precision, bool trace);   // pt_sweep_group.cu
+PtSweepFn pt_lookup_cta(int precision, bool trace);                        // pt_sweep_group.cu
+PtSweepFn pt_lookup_comp(const int nik[4], int precision, bool trace);     // pt_sweep_comp*.cu
+// the unrolled variants of k_sweep_group: smallest NI >= ni_needed for this lane count, 0 = run-time loop
+int pt_group_variant(int lanes, int ni_needed);
+// the instantiated (N8, N10, N16, N32) class that covers chain length N with the fewest padded slots; `seven`:
+// the composition is 7 chains on every sub-partition, for which k_sweep_seven (class (N8, N10, -1, -1)) is
+// preferred where it is instantiated for exactly this N; false = no class
+bool pt_comp_class(int N, bool seven, int nik[4]);
+
 
 // pt_sweep.cu
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan);

@@ -1,664 +1,136 @@
-// Metropolis sweep kernels for sm_100a.
-//
-// One chain's coordinates stay in shared memory for the whole launch (SoA x[], y[], z[]).
-// Inside a chain the Markov chain is strictly serial; the parallelism is
-//   (i)  over partner monomers j of the moved monomer m: L lanes stride over j and each adds
-//        E_LJ^mod(|x' - x_j|) - E_LJ^mod(|x_m - x_j|) for its partners (Eq. 1, 2, 5), and
-//   (ii) over chains: 32/L chains per warp, so that the serial part of a step (Philox, the FENE
-//        sqrt/log, the Metropolis exp) is one instruction stream shared by 32/L chains.
-// The paper's kernel (Listing 2) maps one replica to one block of 64 threads and
-// recomputes the whole energy; that is prior art, kept only as the CTA-per-replica variant for
-// very long chains (N > 480), and with the local Delta-E of Eq. (5) instead of the full sum.
-//
-// Kernels: k_sweep_group (L = 8, 16, 32 lanes per chain, partner loop unrolled in stage-major groups
-// with the bond stream interleaved), k_sweep_mixed (8- and 10-lane warps side by side against wave
-// quantisation), k_sweep_cta.  pt_plan_sweep chooses; DESIGN.md section 7 has the measurements.
-#include <math.h>
+// Host side of the sweep kernels: which kernel and which mapping of chains to warps (pt_plan_sweep), and the
+// launch.  The kernels themselves live in pt_sweep_kernels.cuh and are instantiated in pt_sweep_group.cu
+// (uniform warps, one CTA per replica) and pt_sweep_comp<u>.cu (composed CTAs).  DESIGN.md section 7 has the
+// measurements behind the rules.
 #include <stdio.h>
 
-#include "pt_sweep_common.cuh"
+#include "pt_internal.h"
+#include "pt_sweep_classes.h"
 
-namespace {
+// one lookup per translation unit of pt_sweep_classes.h
+#define PT_DECL(u) PtSweepFn pt_lookup_comp_##u(const int nik[4], int precision, bool trace);
+PT_DECL(0) PT_DECL(1) PT_DECL(2) PT_DECL(3) PT_DECL(4) PT_DECL(5) PT_DECL(6) PT_DECL(7)
+#undef PT_DECL
+static_assert(PT_COMP_UNITS == 8, "declare and call the lookup of every unit");
 
-// A2 for eight steps at once.  All lanes of a chain would draw the same Philox block; instead lane l
-// (mod 8) draws the block of step g0 + l, converts it to the displacement (width * s, one rounding,
-// DESIGN.md R7) and the acceptance uniform, and every step fetches its four numbers with shuffles:
-// 1/8 of the integer work per step.  Steps are numbered g = sweep * N + k within the launch.
-template <typename Real> struct DrawBlock {
-  Real dx, dy, dz, u;
-  int m;
-};
-
-template <typename Real>
-__device__ __forceinline__ DrawBlock<Real> draw_block(const ChainCtx& c, bool pick, int N, Real width, uint32_t t0,
-                                                      int g0, int lig)
+PtSweepFn pt_lookup_comp(const int nik[4], int precision, bool trace)
 {
-  const int gl = g0 + (lig & 7);
-  const uint32_t k = (uint32_t)(gl % N), t = t0 + (uint32_t)(gl / N);
-  DrawBlock<Real> b;
-  b.m = (int)k;
-  if (pick) {   // "a random monomer of the chain is picked"
-    const uint4 wp = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_PICK, (uint32_t)c.i);
-    b.m = (int)__umulhi(wp.x, (uint32_t)N);
-  }
-  const uint4 w = pt_draw(c.key, k, t, (uint32_t)c.e, PT_TAG_MOVE, (uint32_t)c.i);
-  b.dx = PtNum<Real>::scale(width, PtNum<Real>::sym(w.x));
-  b.dy = PtNum<Real>::scale(width, PtNum<Real>::sym(w.y));
-  b.dz = PtNum<Real>::scale(width, PtNum<Real>::sym(w.z));
-  b.u = PtNum<Real>::u01(w.w);
-  return b;
-}
-
-template <typename Real>
-__device__ __forceinline__ DrawBlock<Real> draw_fetch(const DrawBlock<Real>& b, int g, unsigned gsh)
-{
-  const int src = (int)gsh + (g & 7);
-  DrawBlock<Real> r;
-  r.dx = __shfl_sync(0xffffffffu, b.dx, src);
-  r.dy = __shfl_sync(0xffffffffu, b.dy, src);
-  r.dz = __shfl_sync(0xffffffffu, b.dz, src);
-  r.u = __shfl_sync(0xffffffffu, b.u, src);
-  r.m = __shfl_sync(0xffffffffu, b.m, src);
-  return r;
-}
-
-// A5 + the logarithm of A6 (same roles and arithmetic as bonds_and_logu) cut into LEVELS of mutually
-// independent instructions.  A warp issues in order: as one block of code these ~30 dependent fp64
-// levels run back to back at the full 8-cycle DFMA latency (the S of DESIGN.md section 7, about 40 %
-// of a one-warp step).  The pair groups call run<P, NPTS>() after each of their stages instead: one
-// dependent level per ~10 independent pair instructions.  The logarithm's series is evaluated by
-// Estrin's scheme (depth 4 instead of 10).
-template <typename Real> struct BondChain {
-  static constexpr int NLEV = 31;
-  const PtDev& d;
-  const PtCoords<Real>& X;
-  int role, m, N;
-  Real xo, yo, zo, xn, yn, zn, u;
-  // results
-  Real bond, lg;
-  bool broke;
-  // intermediates
-  Real xb, yb, zb, dx, dy, dz, r2, r, q, gq;
-  Real y, g, h, rr, tt;
-  Real f, mp, x, e, sv, s2, z, z2, z4, z8, p01, p23, p45, p67, p89, q0, q1, pz, de;
-  bool isbond, isnew, in_range;
-
-  __device__ __forceinline__ BondChain(const PtDev& dev, const PtCoords<Real>& coords) : d(dev), X(coords) {}
-
-  template <int K> __device__ __forceinline__ void level()
-  {
-    if (K == 0) {
-      const int nb = (role & 1) ? m + 1 : m - 1;
-      isbond = role < 4 && nb >= 0 && nb < N;
-      isnew = role < 2;
-      X.get(isbond ? nb : m, xb, yb, zb);
-    }
-    if (K == 1) {
-      dx = (isnew ? xn : xo) - xb;
-      dy = (isnew ? yn : yo) - yb;
-      dz = (isnew ? zn : zo) - zb;
-    }
-    if (K == 2) r2 = dx * dx;
-    if (K == 3) r2 = fma(dy, dy, r2);
-    if (K == 4) { r2 = fma(dz, dz, r2); r2 = isbond ? r2 : (Real)(d.r0 * d.r0); }
-    if constexpr (sizeof(Real) == 8) {
-      // sqrt: MUFU.RSQ64H seed y, g = a y, r = (1 - a y^2)/2, sqrt a = g (1 + r + 3/2 r^2)
-      if (K == 5) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-      if (K == 6) { g = r2 * y; h = 0.5 * y; }
-      if (K == 7) rr = fma(-h, g, 0.5);
-      if (K == 8) tt = 1.5 * rr;
-      if (K == 9) tt = fma(tt, rr, rr);
-      if (K == 10) r = fma(g, tt, g);
-    } else {
-      if (K == 5) r = sqrtf(r2);
-    }
-    if (K == 11) q = r - (Real)d.r0;
-    if (K == 12) q = q * (Real)d.invR;
-    if (K == 13) gq = fma(-q, q, (Real)1);               // 1 - ((r - r0)/R)^2, Eq. (3)
-    if (K == 14) {
-      in_range = gq > (Real)0;                           // false for NaN as well
-      broke = isbond && isnew && !in_range;
-      gq = role == 4 ? u : ((isbond && in_range) ? gq : (Real)1);   // argument of the logarithm
-    }
-    if constexpr (sizeof(Real) == 8) {
-      // log v, v = 2^e m, m in [sqrt(1/2), sqrt(2)): log m = 2 atanh(s), s = (m-1)/(m+1) (PtNum<double>::log_)
-      if (K == 15) {
-        const int hi = __double2hiint(gq);
-        const int ex = (hi - 0x3fe6a09e) >> 20;
-        const double mm = __hiloint2double(hi - (ex << 20), __double2loint(gq));
-        de = (double)ex;
-        f = mm - 1.0;
-        mp = mm + 1.0;
-      }
-      if (K == 16) x = PtNum<double>::rcp_seed(mp);
-      if (K == 17) e = fma(-mp, x, 1.0);
-      if (K == 18) e = fma(e, e, e);
-      if (K == 19) x = fma(x, e, x);
-      if (K == 20) sv = f * x;
-      if (K == 21) { z = sv * sv; s2 = sv + sv; }
-      if (K == 22) {
-        p01 = fma(kPtLogC[1], z, kPtLogC[0]);
-        p23 = fma(kPtLogC[3], z, kPtLogC[2]);
-        p45 = fma(kPtLogC[5], z, kPtLogC[4]);
-        p67 = fma(kPtLogC[7], z, kPtLogC[6]);
-        p89 = fma(kPtLogC[9], z, kPtLogC[8]);
-        z2 = z * z;
-      }
-      if (K == 23) { q0 = fma(p23, z2, p01); q1 = fma(p67, z2, p45); z4 = z2 * z2; }
-      if (K == 24) { q0 = fma(q1, z4, q0); z8 = z4 * z4; }
-      if (K == 25) q0 = fma(p89, z8, q0);
-      if (K == 26) pz = q0 * z;
-      if (K == 27) lg = fma(sv, pz, s2);
-      if (K == 28) lg = fma(de, 0x1.abc9e3b39803fp-56, lg);
-      if (K == 29) lg = fma(de, 0x1.62e42fefa39efp-1, lg);
-    } else {
-      if (K == 15) lg = __logf(gq);
-    }
-    if (K == 30) bond = role < 4 ? (isnew ? (Real)d.feneC : (Real)-d.feneC) * lg : (Real)0;
-  }
-  template <int A, int B> __device__ __forceinline__ void range()
-  {
-    if constexpr (A < B) {
-      level<A>();
-      range<A + 1, B>();
-    }
-  }
-  // stage point P of NPTS
-  // stage point P of NPTS; LEVG = levels handed out over the stage points (the rest runs after the pair groups)
-  template <int P, int NPTS, int LEVG> __device__ __forceinline__ void run()
-  {
-    range<(P * LEVG) / NPTS, ((P + 1) * LEVG) / NPTS>();
-  }
-  __device__ __forceinline__ void run_all() { range<0, NLEV>(); }
-};
-
-constexpr int kGroupPoints = 14;   // stage points per pair group
-
-// A3 for CNT partner iterations at once (iterations BEGIN .. BEGIN+CNT-1 of this lane), written stage
-// by stage across the partners: every stage holds CNT or 2 CNT independent fp64 instructions, so that
-// a dependent instruction is not issued within the 8-cycle DFMA latency of its producer (written
-// partner by partner, ptxas kept one or two chains in flight).
-//
-// Arithmetic (Eq. 1-2).  With u = 1/r^6 and c = B/A, E_LJ^mod = A u (u - c) - C inside the cutoff.
-// Per evaluation v = u - c/2 (one DFMA from x^2 and x = 1/r^2); per partner
-//   u_n (u_n - c) - u_o (u_o - c) = (v_n - v_o)(v_n + v_o):   DADD, DADD, DFMA.
-// A pair outside the cutoff, and the moved monomer itself, get a zero reciprocal seed (one FSEL), which stays
-// zero through the Newton step: u = 0, v = -c/2, and the partner adds exactly nothing unless it crosses the
-// cutoff.  The cutoff test is one DSETP (fp64 pipe) with the "not myself" mask as its predicate input, the
-// shift C needs the count of inside pairs (one predicated add); A and C are applied once per step by the
-// caller.  The new squared distance follows from the old one:
-// |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
-template <typename Real, int L, int NI, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
-__device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
-                                           Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
-                                           Real (&acc)[4], int& cnt, BondChain<Real>& side)
-{
-#define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
-  Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) X.get(s0 + (BEGIN + u) * L, bx[u], by[u], bz[u]);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) { bx[u] = xo - bx[u]; by[u] = yo - by[u]; bz[u] = zo - bz[u]; }
-  PT_SIDE(0);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = bx[u] * bx[u];
-  PT_SIDE(1);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = fma(by[u], by[u], ro[u]);
-  PT_SIDE(2);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = fma(bz[u], bz[u], ro[u]);
-  PT_SIDE(3);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + dd;
-  PT_SIDE(4);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdz, bz[u], rn[u]);
-  PT_SIDE(5);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdy, by[u], rn[u]);
-  PT_SIDE(6);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdx, bx[u], rn[u]);
-  PT_SIDE(7);
-  Real dv[2 * CNT], xv[2 * CNT], ev[2 * CNT];
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) {
-    const int j = s0 + (BEGIN + u) * L;
-    dv[2 * u] = ro[u];
-    dv[2 * u + 1] = rn[u];
-    xv[2 * u] = PtNum<Real>::template seed_if_inside<-1>(ro[u], lj.rc2, j, sm, cnt);
-    xv[2 * u + 1] = PtNum<Real>::template seed_if_inside<1>(rn[u], lj.rc2, j, sm, cnt);
-  }
-  PT_SIDE(8);
-  if (PtNum<Real>::kNewton) {
-#pragma unroll
-    for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(-dv[v], xv[v], (Real)1);
-    PT_SIDE(9);
-#pragma unroll
-    for (int v = 0; v < 2 * CNT; ++v) ev[v] = fma(ev[v], ev[v], ev[v]);
-    PT_SIDE(10);
-#pragma unroll
-    for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(xv[v], ev[v], xv[v]);
-  } else {   // fp32: the MUFU reciprocal is final; the serial stream still gets its two turns
-    PT_SIDE(9);
-    PT_SIDE(10);
-  }
-#pragma unroll
-  for (int v = 0; v < 2 * CNT; ++v) ev[v] = xv[v] * xv[v];
-  PT_SIDE(11);
-#pragma unroll
-  for (int v = 0; v < 2 * CNT; ++v) xv[v] = fma(ev[v], xv[v], lj.mhc);          // v = 1/r^6 - c/2
-  PT_SIDE(12);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) {
-    ev[2 * u] = xv[2 * u + 1] - xv[2 * u];
-    ev[2 * u + 1] = xv[2 * u + 1] + xv[2 * u];
-  }
-  PT_SIDE(13);
-#pragma unroll
-  for (int u = 0; u < CNT; ++u) acc[(BEGIN + u) & 3] = fma(ev[2 * u], ev[2 * u + 1], acc[(BEGIN + u) & 3]);
-#undef PT_SIDE
-}
-
-// How the NI partner iterations of a lane are cut into groups (each group is one stage-major block of
-// pair_group).  Balanced groups of at most kMaxGroup partners: 13 -> 5 + 4 + 4, 10 -> 5 + 5, <= 5 -> one group.
-// Measured on B200 (config 5): 5 + 4 + 4 / 5 + 5 is 3 % faster than 4 + 4 + 5 / 4 + 6.
-#ifndef PT_MAXGROUP
-#define PT_MAXGROUP 5
-#endif
-constexpr int kMaxGroup = PT_MAXGROUP;
-__host__ __device__ constexpr int n_groups(int NI) { return NI <= 0 ? 0 : (NI + kMaxGroup - 1) / kMaxGroup; }
-// size and first iteration of group g: the first (NI mod n) groups get one more
-__host__ __device__ constexpr int group_size(int NI, int g) { return NI / n_groups(NI) + (g < NI % n_groups(NI) ? 1 : 0); }
-__host__ __device__ constexpr int group_begin(int NI, int g) { return g == 0 ? 0 : group_begin(NI, g - 1) + group_size(NI, g - 1); }
-
-// The whole partner loop of NI > 0 iterations: returns this lane's share of Delta E_LJ.
-// s0 = this lane's first partner, sm = the moved monomer (its own slot is masked out).
-template <typename Real, int L, int NI, int LEVG>
-__device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
-                                            Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
-                                            BondChain<Real>& side)
-{
-  constexpr int P = kGroupPoints;
-  constexpr int NG = n_groups(NI);
-  static_assert(NG >= 1 && NG <= 4, "add a group");
-  Real acc[4] = {(Real)0, (Real)0, (Real)0, (Real)0};
-  int cnt = 0;
-#define PT_PG(g)                                                                                             \
-  if (NG > g)                                                                                                \
-    pair_group<Real, L, NI, group_begin(NI, g < NG ? g : 0), group_size(NI, g < NG ? g : 0), g * P, NG * P, LEVG>( \
-        lj, X, s0, sm, xo, yo, zo, tdx, tdy, tdz, dd, acc, cnt, side)
-  PT_PG(0);
-  PT_PG(1);
-  PT_PG(2);
-  PT_PG(3);
-#undef PT_PG
-  return fma(lj.A, (acc[0] + acc[1]) + (acc[2] + acc[3]), -lj.C * (Real)cnt);
-}
-
-// ------------------------------------------------------------------------------------------
-// Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
-// ------------------------------------------------------------------------------------------
-// NI > 0: the partner loop has exactly NI iterations (Ns = NI * L) and is unrolled completely, so
-// that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
-// pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
-// One warp's share of a sweep launch: G = 32 / L chains starting at slot `chain0`, coordinates at
-// `smem0` (stride `sstride` Reals between chains, Ns slots per coordinate array).  `delay`: cycles to
-// wait before the first step (phase stagger).
-template <typename Real, int L, int NI, bool TRACE>
-__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns, int chain0, int delay,
-                                           const uint32_t t0, const int n_sweeps)
-{
-  static_assert(L >= 8 && L <= 32, "lanes per chain");
-  constexpr int G = 32 / L;
-  // Short partner loops have fewer stage points than the bond stream has levels: one level per point,
-  // the rest of the stream runs behind the reduction of the pair sums (latency-bound shapes).
-  constexpr int NPTS = n_groups(NI) * kGroupPoints;
-  constexpr bool TAIL = NI > 0 && (L & (L - 1)) == 0 && NPTS < BondChain<Real>::NLEV;
-  constexpr int LEVG = TAIL ? NPTS : BondChain<Real>::NLEV;
-  // lanes beyond G L (L = 10: lanes 30, 31) are ghosts: they repeat the last real lane and nobody reads them
-  const int lane = min((int)(threadIdx.x & 31), G * L - 1);
-  const int g = lane / L, lig = lane % L;
-  const int gbase = g * L;
-  const int N = d.N;
-
-  ChainCtx c;
-  ctx_load(d, chain0 + g, c);
-  const Real width = (Real)d.width[c.i];
-  const PtLJ<Real> lj(d);
-
-  const PtCoords<Real> X(smem0 + (size_t)g * sstride, Ns);
-
-  // A1: HBM -> shared memory; padding entries lie far outside every cutoff
-  Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
-  for (int j = lig; j < Ns; j += L) {
-    const bool in = j < N;
-    X.set(j, in ? gx[j] : (Real)PT_FAR, in ? gx[d.Ng + j] : (Real)PT_FAR, in ? gx[2 * d.Ng + j] : (Real)PT_FAR);
-  }
-  __syncwarp();
-
-  if (delay > 0) {
-    const long long until = clock64() + (long long)delay;
-    while (clock64() < until) { }
-  }
-
-  const bool pick = d.select_mode == PT_RANDOM_PICK;
-  const bool leader = (lig == 0) && c.active;
-  const unsigned bond_lanes = 3u << gbase;   // roles 0, 1 of this group: the new bonds
-  const double nbeta = -c.beta;
-
-  const unsigned gsh = (unsigned)gbase;
-  DrawBlock<Real> blk = draw_block<Real>(c, pick, N, width, t0, 0, lig);
-  DrawBlock<Real> nx = draw_fetch<Real>(blk, 0, gsh);
-  int gstep = 0;   // step number within the launch
-  for (int sw = 0; sw < n_sweeps; ++sw) {
-    const uint32_t t = t0 + (uint32_t)sw;
-    for (int k = 0; k < N; ++k) {
-      // A2: this step's numbers were fetched one step ahead; fetch the next ones now (and draw the
-      // next eight blocks when they are used up) so that the shuffles overlap the fp64 work below
-      const DrawBlock<Real> p = nx;
-      ++gstep;
-      if ((gstep & 7) == 0) blk = draw_block<Real>(c, pick, N, width, t0, gstep, lig);
-      nx = draw_fetch<Real>(blk, gstep, gsh);
-      const int m = p.m;
-      Real xo, yo, zo;
-      X.get(m, xo, yo, zo);
-      const Real xn = PtNum<Real>::shift(xo, p.dx);
-      const Real yn = PtNum<Real>::shift(yo, p.dy);
-      const Real zn = PtNum<Real>::shift(zo, p.dz);
-      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
-      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
-      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
-
-      // A5 (bonds, and log u of A6) rides along with A3 (Delta E_LJ, lanes stride over partners, Eq. 1, 2)
-      BondChain<Real> bc(d, X);
-      bc.role = lig; bc.m = m; bc.N = N;
-      bc.xo = xo; bc.yo = yo; bc.zo = zo; bc.xn = xn; bc.yn = yn; bc.zn = zn; bc.u = p.u;
-      Real part;
-      if (NI > 0) {
-        part = pair_groups<Real, L, (NI > 0 ? NI : 1), LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
-      } else {
-        bc.run_all();
-        Real en = (Real)0, eo = (Real)0;
-        int cnt = 0;
-#pragma unroll 2
-        for (int j = lig; j < Ns; j += L)
-          pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
-        part = fma(-lj.C, (Real)cnt, en - eo);
-      }
-      Real dE, logu;
-      bool bond_broken;
-      if (TAIL) {
-        // A4 in two parts: the pair sums are reduced while the bond stream finishes (its last levels ride
-        // on the shuffle latencies); the bond terms sit in lanes 0..3 of the group and need two levels
-        Real v = part;
-        constexpr int REM = BondChain<Real>::NLEV - LEVG;
-        constexpr int NSH = L == 32 ? 5 : (L == 16 ? 4 : 3);
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-        bc.template range<LEVG, LEVG + REM / NSH>();
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        bc.template range<LEVG + REM / NSH, LEVG + 2 * REM / NSH>();
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        bc.template range<LEVG + 2 * REM / NSH, LEVG + 3 * REM / NSH>();
-        if (L >= 16) {
-          v += __shfl_xor_sync(0xffffffffu, v, 8);
-          bc.template range<LEVG + 3 * REM / NSH, LEVG + 4 * REM / NSH>();
-        }
-        if (L == 32) {
-          v += __shfl_xor_sync(0xffffffffu, v, 16);
-          bc.template range<LEVG + 4 * REM / NSH, LEVG + REM>();
-        }
-        Real b = bc.bond;
-        b += __shfl_xor_sync(0xffffffffu, b, 1);
-        b += __shfl_xor_sync(0xffffffffu, b, 2);
-        bond_broken = (__ballot_sync(0xffffffffu, bc.broke) & bond_lanes) != 0u;
-        logu = __shfl_sync(0xffffffffu, bc.lg, gbase + 4);
-        dE = v + __shfl_sync(0xffffffffu, b, gbase);
-      } else {
-        bond_broken = (__ballot_sync(0xffffffffu, bc.broke) & bond_lanes) != 0u;
-        logu = __shfl_sync(0xffffffffu, bc.lg, gbase + 4);
-        // A4: reduce; every lane of the group gets the same Delta E
-        dE = group_sum<Real, L>(part + bc.bond, lig, gbase);
-      }
-
-      // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
-      const bool accept = !bond_broken && (dE <= (Real)0 || (double)logu < nbeta * (double)dE);
-
-      // A7: commit (branch-free: predicated stores, selects for the bookkeeping)
-      if (accept && lig == 0) X.set(m, xn, yn, zn);
-      if (TRACE) {   // test support (pt_set_trace): a separate instantiation, the timed one has no branch here
-        if (lig == 0 && d.tr_move && c.active && (long long)t < d.cap_sweeps)
-          d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
-      }
-      c.erun += accept ? (double)dE : 0.0;
-      c.acc += accept ? 1u : 0u;
-      c.brej += bond_broken ? 1u : 0u;
-      __syncwarp();
-    }
-
-    // A8: measurement once per sweep
-    if (d.observables) measure_shape<Real, L>(d, c, N, lig, gbase, X);
-    if (leader) measure_energy(d, c, t);
-  }
-
-  // A9: shared memory -> HBM
-  __syncwarp();
-  if (c.active) {
-    for (int j = lig; j < N; j += L) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
-    if (lig == 0) ctx_store(d, c, n_sweeps);
-  }
-}
-
-// Warps w and w + 4 of a CTA share an SM sub-partition and run the same code: started together they
-// stay in phase, both in the fp64-bound pair loop, then both in the latency-bound serial part of
-// the step (period 2P + S).  The second one therefore starts `stagger` cycles (about one partner
-// loop) late, so that its serial part can hide under the pair loop of the first.
-template <typename Real, int L, int NI, bool TRACE>
-__global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtLaunch pl, const uint32_t t0,
-                                                     const int n_sweeps)
-{
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  constexpr int G = 32 / L;
-  const int warp = threadIdx.x >> 5;
-  sweep_warp<Real, L, NI, TRACE>(d, reinterpret_cast<Real*>(smem_raw) + (size_t)(warp * G) * pl.sstride, pl.sstride, pl.Ns,
-                                 blockIdx.x * pl.chains_per_cta + warp * G, pl.stagger * (warp >> 2), t0, n_sweeps);
-}
-
-// Mixed mapping against wave quantisation (the paper's staircase): when the chains
-// per sub-partition lie between 4 and 7, uniform 4-chain warps leave sub-partitions with two warps
-// (8 chains) next to sub-partitions with one.  Here every sub-partition gets 7 chains: one warp of
-// 4 chains x 8 lanes (13 partner iterations) and one warp of 3 chains x 10 lanes (10 iterations, lanes
-// 30, 31 idle), 28 chains per CTA of 8 warps.  NA, NB = partner iterations of the two kinds of warp
-// (8 NA and 10 NB slots >= N); instantiated for the shapes listed in kMixed.
-template <typename Real, int NA, int NB, bool TRACE>
-__global__ void __launch_bounds__(256, 1) k_sweep_mixed(const PtDev d, const PtLaunch pl, const uint32_t t0,
-                                                     const int n_sweeps)
-{
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  Real* base = reinterpret_cast<Real*>(smem_raw);
-  const int warp = threadIdx.x >> 5;
-  const int cta0 = blockIdx.x * 28;
-  if (warp < 4)
-    sweep_warp<Real, 8, NA, TRACE>(d, base + (size_t)(warp * 4) * pl.sstride, pl.sstride, 8 * NA, cta0 + warp * 4, 0, t0,
-                                   n_sweeps);
-  else
-    sweep_warp<Real, 10, NB, TRACE>(d, base + (size_t)16 * pl.sstride + (size_t)((warp - 4) * 3) * pl.sstride2,
-                                    pl.sstride2, 10 * NB, cta0 + 16 + (warp - 4) * 3, pl.stagger, t0, n_sweeps);
-}
-
-struct MixedVariant {
-  int NA, NB;
-  PtSweepFn f64[2], f32[2];   // [0] timed, [1] with the decision trace
-};
-#define PT_MIXED(NA, NB)                                                                     \
-  { NA, NB, { k_sweep_mixed<double, NA, NB, false>, k_sweep_mixed<double, NA, NB, true> },   \
-    { k_sweep_mixed<float, NA, NB, false>, k_sweep_mixed<float, NA, NB, true> } }
-// N = 51..56 (the paper's N = 55) and N = 97..100 (the throughput batch)
-#ifdef PT_FEW_VARIANTS
-const MixedVariant kMixed[] = { PT_MIXED(13, 10) };
-#else
-const MixedVariant kMixed[] = { PT_MIXED(7, 6), PT_MIXED(13, 10) };
-#endif
-
-const MixedVariant* find_mixed(int N)
-{
-  for (const MixedVariant& v : kMixed)
-    if ((N + 7) / 8 == v.NA && (N + 9) / 10 == v.NB) return &v;
+  PtSweepFn (*const units[])(const int*, int, bool) = {pt_lookup_comp_0, pt_lookup_comp_1, pt_lookup_comp_2,
+                                                       pt_lookup_comp_3, pt_lookup_comp_4, pt_lookup_comp_5,
+                                                       pt_lookup_comp_6, pt_lookup_comp_7};
+  for (auto f : units)
+    if (PtSweepFn k = f(nik, precision, trace)) return k;
   return nullptr;
 }
 
-// ------------------------------------------------------------------------------------------
-// CTA-per-replica kernel: blockDim.x threads share one chain (long chains, few replicas).
-// ------------------------------------------------------------------------------------------
-template <typename Real, bool TRACE>
-__global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLaunch pl, const uint32_t t0,
-                                                   const int n_sweeps)
-{
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ double red[2][8];
-  __shared__ double s_logu[2];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int T = blockDim.x, NW = T >> 5;
-  const int N = d.N, Ns = pl.Ns;
+namespace {
 
-  ChainCtx c;
-  ctx_load(d, blockIdx.x, c);
-  const Real width = (Real)d.width[c.i];
-  const PtLJ<Real> lj(d);
+struct CompClass { int nik[4]; };
+#define PT_COMP(A, B, C, D) {{A, B, C, D}},
+#define PT_SEVEN(A, B) {{A, B, -1, -1}},
+const CompClass kCompClasses[] = {PT_COMP_CLASSES_0 PT_COMP_CLASSES_1 PT_COMP_CLASSES_2 PT_COMP_CLASSES_3
+                                  PT_COMP_CLASSES_4 PT_COMP_CLASSES_5 PT_COMP_CLASSES_6 PT_COMP_CLASSES_7};
+#undef PT_COMP
+#undef PT_SEVEN
 
-  const PtCoords<Real> X(reinterpret_cast<Real*>(smem_raw), Ns);
-  Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
-  for (int j = tid; j < Ns; j += T) {
-    const bool in = j < N;
-    X.set(j, in ? gx[j] : (Real)PT_FAR, in ? gx[d.Ng + j] : (Real)PT_FAR, in ? gx[2 * d.Ng + j] : (Real)PT_FAR);
-  }
-  __syncthreads();
-
-  const bool pick = d.select_mode == PT_RANDOM_PICK;
-  const double nbeta = -c.beta;
-  Proposal<Real> nx = draw_proposal<Real>(c, pick, N, 0u, t0);
-  for (int sw = 0; sw < n_sweeps; ++sw) {
-    const uint32_t t = t0 + (uint32_t)sw;
-    for (int k = 0; k < N; ++k) {
-      const Proposal<Real> p = nx;
-      {
-        const bool last = k + 1 == N;
-        nx = draw_proposal<Real>(c, pick, N, last ? 0u : (uint32_t)(k + 1), last ? t + 1u : t);
-      }
-      const int m = p.m;
-      Real xo, yo, zo;
-      X.get(m, xo, yo, zo);
-      const Real xn = PtNum<Real>::propose(xo, width, p.sx);
-      const Real yn = PtNum<Real>::propose(yo, width, p.sy);
-      const Real zn = PtNum<Real>::propose(zo, width, p.sz);
-      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
-      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
-      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
-
-      Real en = (Real)0, eo = (Real)0;
-      int cnt = 0;
-#pragma unroll 2
-      for (int j = tid; j < Ns; j += T)
-        pair_terms<Real>(lj, j != m, X, j, xo, yo, zo, tdx, tdy, tdz, dd, en, eo, cnt);
-      Real part = fma(-lj.C, (Real)cnt, en - eo);
-
-      // bonds and log u: roles 0..4 are threads 0..4 of warp 0; the other warps skip the stream
-      bool broke = false;
-      if (warp == 0) {
-        Real lg;
-        part += bonds_and_logu<Real>(d, lane, m, N, X, xo, yo, zo, xn, yn, zn, p.u, &lg, &broke);
-        if (lane == 4) s_logu[k & 1] = (double)lg;
-      }
-      const Real wsum = group_sum<Real, 32>(part, lane, 0);
-      if (lane == 0) red[k & 1][warp] = (double)wsum;
-      const bool bond_broken = __syncthreads_or(broke ? 1 : 0) != 0;
-      double dEd = red[k & 1][0];
-      for (int q = 1; q < NW; ++q) dEd += red[k & 1][q];
-      const Real dE = (Real)dEd;
-      const double logu = s_logu[k & 1];
-
-      const bool accept = !bond_broken && (dE <= (Real)0 || logu < nbeta * (double)dE);
-
-      if (tid == 0) {
-        if (accept) X.set(m, xn, yn, zn);
-        if (TRACE) {   // test support (pt_set_trace): a separate instantiation
-          if (d.tr_move && (long long)t < d.cap_sweeps)
-            d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
-        }
-      }
-      if (accept) { c.erun += (double)dE; c.acc++; }
-      c.brej += bond_broken ? 1u : 0u;
-      __syncthreads();
-    }
-
-    if (d.observables && warp == 0) measure_shape<Real, 32>(d, c, N, lane, 0, X);
-    if (tid == 0) measure_energy(d, c, t);
-  }
-
-  __syncthreads();
-  for (int j = tid; j < N; j += T) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
-  if (tid == 0) ctx_store(d, c, n_sweeps);
-}
+const int kLanesOfKind[4] = {8, 10, 16, 32};
+const int kChainsOfKind[4] = {4, 3, 2, 1};
 
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 constexpr int kSmemCap = 200 * 1024;   // dynamic shared memory any sweep kernel may ask for
 
-typedef PtSweepFn SweepFn;
-
-struct SweepVariant {
-  int L, NI;
-  SweepFn f64[2], f32[2];   // [0] timed, [1] with the decision trace
-};
-
-#define PT_VARIANT(L, NI)                                                              \
-  { L, NI, { k_sweep_group<double, L, NI, false>, k_sweep_group<double, L, NI, true> }, \
-    { k_sweep_group<float, L, NI, false>, k_sweep_group<float, L, NI, true> } }
-// Unrolled instantiations (NI = partner-loop iterations); NI = 0 is the run-time loop of the same
-// lane count and must come last within its L.
-const SweepVariant kVariants[] = {
-#ifdef PT_FEW_VARIANTS
-    PT_VARIANT(8, 13), PT_VARIANT(8, 0), PT_VARIANT(16, 1), PT_VARIANT(16, 0), PT_VARIANT(32, 1), PT_VARIANT(32, 2),
-    PT_VARIANT(32, 10), PT_VARIANT(32, 0),
-#else
-    PT_VARIANT(8, 2),  PT_VARIANT(8, 4),  PT_VARIANT(8, 7),  PT_VARIANT(8, 10), PT_VARIANT(8, 13),
-    PT_VARIANT(8, 0),
-    PT_VARIANT(16, 1), PT_VARIANT(16, 2), PT_VARIANT(16, 4), PT_VARIANT(16, 7), PT_VARIANT(16, 0),
-    PT_VARIANT(32, 1), PT_VARIANT(32, 2), PT_VARIANT(32, 4), PT_VARIANT(32, 7), PT_VARIANT(32, 10),
-    PT_VARIANT(32, 13), PT_VARIANT(32, 15), PT_VARIANT(32, 0),
-#endif
-};
-
-const SweepVariant* find_variant(int L, int ni_needed)
+// Chains of one warp must start in different banks: stride = L (mod Q) words, where Q words span all 32
+// banks (fp64: a warp's 8-byte loads go in two phases of 16 lanes, Q = 16).
+int chain_stride(int Ns, int L, int real_bytes)
 {
-  for (const SweepVariant& v : kVariants)
-    if (v.L == L && (v.NI == 0 || v.NI >= ni_needed)) return &v;
-  return nullptr;
+  const int Q = 128 / real_bytes;
+  int ss = 3 * Ns;
+  while (ss % Q != L % Q) ++ss;
+  return ss;
 }
 
-SweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
+// phase stagger between two warps of the same kind on one sub-partition: about the fp64 time of one partner loop
+int stagger_cycles(int ni) { return (int)(2.1 * (26.0 * ni + 70.0)); }
+
+PtSweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
-  if (pl.kind == PT_K_CTA) {
-    if (precision == PT_F32) return trace ? (SweepFn)k_sweep_cta<float, true> : (SweepFn)k_sweep_cta<float, false>;
-    return trace ? (SweepFn)k_sweep_cta<double, true> : (SweepFn)k_sweep_cta<double, false>;
+  if (pl.kind == PT_K_CTA) return pt_lookup_cta(precision, trace);
+  if (pl.kind == PT_K_COMP) return pt_lookup_comp(pl.nik, precision, trace);
+  return pt_lookup_group(pl.lanes, pl.ni, precision, trace);
+}
+
+// Composed CTAs (k_sweep_comp): chains spread evenly over the SMs, one CTA per SM and wave, every sub-partition
+// one or two warps chosen for its load.  Returns false if this shape is not covered.
+bool plan_comp(const PtDev& d, int real_bytes, int sms, PtLaunch* out)
+{
+  PtLaunch pl{};
+  const long long cap = 32ll * sms;                       // 8 chains per sub-partition: two warps of 4
+  const long long waves = (d.C + cap - 1) / cap;
+  const int q = (int)((d.C + sms * waves - 1) / (sms * waves));   // chains per CTA
+  // kinds of the (at most) two warps of a sub-partition that holds `load` chains; -1 = no warp
+  static const int kWarps[9][2] = {{-1, -1}, {3, -1}, {2, -1}, {1, -1}, {0, -1}, {1, 2}, {1, 1}, {0, 1}, {0, 0}};
+  if (!pt_comp_class(d.N, q == 28, pl.nik)) return false;
+  pl.kind = PT_K_COMP;
+  pl.chains_per_cta = q;
+  pl.grid = (int)((d.C + q - 1) / q);
+  for (int k = 0; k < 4; ++k)
+    pl.kstride[k] = pl.nik[k] > 0 ? chain_stride(kLanesOfKind[k] * pl.nik[k], kLanesOfKind[k], real_bytes) : 0;
+  int first = 0, off = 0, nwarps = 4, lanes_min = 32;
+  for (int w = 0; w < 8; ++w) {
+    const int sp = w & 3, load = q / 4 + (sp < q % 4 ? 1 : 0);
+    const int k = kWarps[load][w >> 2];
+    if (k < 0) {
+      pl.wkind[w] = 3;
+      pl.wfirst[w] = 1 << 30;        // beyond every chain: the warp leaves at once
+      continue;
+    }
+    if (w >= 4) nwarps = 8;
+    pl.wkind[w] = k;
+    pl.wfirst[w] = first;
+    pl.woff[w] = off;
+    pl.wdelay[w] = (w >= 4 && kWarps[load][0] == k) ? stagger_cycles(pl.nik[k]) : 0;
+    first += kChainsOfKind[k];
+    off += kChainsOfKind[k] * pl.kstride[k];
+    if (kLanesOfKind[k] < lanes_min) lanes_min = kLanesOfKind[k];
   }
-  if (pl.kind == PT_K_MIXED) {
-    for (const MixedVariant& v : kMixed)
-      if (v.NA == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
-    return nullptr;
-  }
-  for (const SweepVariant& v : kVariants)
-    if (v.L == pl.lanes && v.NI == pl.ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
-  return nullptr;
+  if (first != q) return false;
+  pl.lanes = lanes_min;
+  pl.ni = pl.nik[0];
+  pl.Ns = 8 * pl.nik[0];
+  pl.threads = 32 * nwarps;
+  pl.smem_bytes = off * real_bytes;
+  *out = pl;
+  return true;
 }
 
 }  // namespace
 
+bool pt_comp_class(int N, bool seven, int nik[4])
+{
+  if (N < 17) return false;
+  const CompClass* best = nullptr;
+  int best_waste = 0;
+  for (const CompClass& c : kCompClasses) {
+    const bool is_seven = c.nik[2] < 0;      // k_sweep_seven: exact fit only, and only for that composition
+    bool ok = is_seven ? seven : true;
+    int waste = is_seven ? -1 : 0;
+    for (int k = 0; k < (is_seven ? 2 : 4); ++k) {
+      const int need = (N + kLanesOfKind[k] - 1) / kLanesOfKind[k];
+      ok = ok && (is_seven ? c.nik[k] == need : c.nik[k] >= need);
+      waste += c.nik[k] - need;
+    }
+    if (ok && (!best || waste < best_waste)) { best = &c; best_waste = waste; }
+  }
+  if (!best) return false;
+  for (int k = 0; k < 4; ++k) nik[k] = best->nik[k];
+  return true;
+}
+
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan)
 {
   const int real_bytes = precision == PT_F32 ? 4 : 8;
-  int sms = 148;
+  int sms = 148;   // B200; the device is asked below
   {
     int dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) {
@@ -668,55 +140,37 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     cudaGetLastError();
   }
   const long long smsp = 4ll * sms;
+  PtLaunch pl{};
+  bool done = false;
   int L = lanes_requested;
   if (L == 0) {
-    // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
-    // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
-    // sub-partition costs more than halving the lanes (measured: profiles/r01_paper_timing.md, the
-    // steps at 592 -> 593 and 1184 -> 1185 replicas).  With more than 4 chains per sub-partition there
-    // is no such choice: 8 lanes, the serial part of a step (proposal, bonds, log u, decision) is then
-    // one instruction stream shared by 4 chains.
-    if (d.N > 15 * 32 && (long long)d.C <= smsp) L = 128;   // beyond the unrolled one-warp variants (15 iterations)
-    else {
-      L = 32;
-      while (L > 8 && ((long long)d.C * L + 31) / 32 > smsp && d.N > L / 2) L /= 2;
-      while (L > 8 && L / 2 >= d.N) L /= 2;
+    // More chains than SM sub-partitions: composed CTAs, chains spread evenly over the SMs (no staircase in
+    // the number of replicas beyond the one of the most loaded sub-partition).
+    if ((long long)d.C > smsp) done = plan_comp(d, real_bytes, sms, &pl);
+    if (!done) {
+      // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
+      // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
+      // sub-partition costs more than halving the lanes (measured: profiles/r01_paper_timing.md).  With more
+      // than 4 chains per sub-partition there is no such choice: 8 lanes, the serial part of a step
+      // (proposal, bonds, log u, decision) is then one instruction stream shared by 4 chains.
+      if (d.N > 15 * 32 && (long long)d.C <= smsp) L = 128;   // beyond the unrolled one-warp variants (15 iterations)
+      else {
+        L = 32;
+        while (L > 8 && ((long long)d.C * L + 31) / 32 > smsp && d.N > L / 2) L /= 2;
+        while (L > 8 && L / 2 >= d.N) L /= 2;
+      }
     }
   }
-  PtLaunch pl{};
-  pl.lanes = L;
-  const MixedVariant* mv = find_mixed(d.N);
-  if (lanes_requested == 0 && L == 8 && mv && (long long)d.C > 4 * smsp && (long long)d.C <= 7 * smsp) {
-    // between 4 and 7 chains per sub-partition: 4 + 3 chains on every one (k_sweep_mixed)
-    const int Q = 128 / real_bytes;
-    pl.kind = PT_K_MIXED;
-    pl.ni = mv->NA;
-    pl.ni2 = mv->NB;
-    pl.Ns = 8 * mv->NA;
-    int ss = 3 * pl.Ns;
-    while (ss % Q != 8 % Q) ++ss;
-    pl.sstride = ss;
-    ss = 3 * 10 * mv->NB;
-    while (ss % Q != 10 % Q) ++ss;
-    pl.sstride2 = ss;
-    pl.threads = 256;
-    pl.chains_per_cta = 28;
-    pl.stagger = 0;   // the two kinds of warp have different periods: a start delay changes nothing (measured)
-    pl.grid = (int)((d.C + 27) / 28);
-    pl.smem_bytes = (16 * pl.sstride + 12 * pl.sstride2) * real_bytes;
+  if (done) {
   } else if (L <= 32) {
     const int G = 32 / L;
-    const SweepVariant* v = find_variant(L, (d.N + L - 1) / L);
-    if (!v) return cudaErrorInvalidValue;
+    const int ni = pt_group_variant(L, (d.N + L - 1) / L);
+    if (ni < 0) return cudaErrorInvalidValue;
+    pl.lanes = L;
     pl.kind = PT_K_GROUP;
-    pl.ni = v->NI;
-    pl.Ns = v->NI > 0 ? v->NI * L : round_up(d.N, L);
-    // chains of one warp must start in different banks: stride = L (mod Q) words, where Q words
-    // span all 32 banks (fp64: a warp's 8-byte loads go in two phases of 16 lanes, Q = 16)
-    const int Q = 128 / real_bytes;
-    int ss = 3 * pl.Ns;
-    while (ss % Q != L % Q) ++ss;
-    pl.sstride = ss;
+    pl.ni = ni;
+    pl.Ns = ni > 0 ? ni * L : round_up(d.N, L);
+    pl.sstride = chain_stride(pl.Ns, L, real_bytes);
     // one CTA per SM when there are enough warps (its warps are dealt round-robin to the four
     // sub-partitions, so they are balanced by construction); single-warp CTAs otherwise
     const long long warps = ((long long)d.C + G - 1) / G;
@@ -727,11 +181,11 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     }
     pl.threads = 32 * wpc;
     pl.chains_per_cta = G * wpc;
-    // phase stagger between the warps of a sub-partition: about the fp64 time of one partner loop
-    pl.stagger = wpc > 4 ? (int)(2.1 * (26.0 * (pl.Ns / L) + 70.0)) : 0;
+    pl.stagger = wpc > 4 ? stagger_cycles(pl.Ns / L) : 0;
     pl.grid = (int)((d.C + pl.chains_per_cta - 1) / pl.chains_per_cta);
     pl.smem_bytes = pl.chains_per_cta * pl.sstride * real_bytes;
   } else {
+    pl.lanes = L;
     pl.kind = PT_K_CTA;
     pl.ni = 0;
     pl.Ns = round_up(d.N, L);
@@ -743,7 +197,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   }
   if (pl.smem_bytes > kSmemCap) return cudaErrorInvalidValue;
   for (int trace = 0; trace < 2; ++trace) {
-    SweepFn fn = kernel_of(pl, precision, trace != 0);
+    PtSweepFn fn = kernel_of(pl, precision, trace != 0);
     if (!fn) return cudaErrorInvalidValue;
     if (pl.smem_bytes > 48 * 1024) {
       // the attribute belongs to the kernel, not to the handle: always the same cap, so that two live
@@ -760,14 +214,17 @@ void pt_sweep_kernel_desc(const PtLaunch& pl, int precision, bool trace, char* b
 {
   const char* real = precision == PT_F32 ? "float" : "double";
   if (pl.kind == PT_K_CTA) snprintf(buf, n, "k_sweep_cta<%s,threads=%d,trace=%d>", real, pl.threads, trace ? 1 : 0);
-  else if (pl.kind == PT_K_MIXED) snprintf(buf, n, "k_sweep_mixed<%s,%d,%d,trace=%d>", real, pl.ni, pl.ni2, trace ? 1 : 0);
+  else if (pl.kind == PT_K_COMP && pl.nik[2] < 0)
+    snprintf(buf, n, "k_sweep_seven<%s,%d,%d,trace=%d>", real, pl.nik[0], pl.nik[1], trace ? 1 : 0);
+  else if (pl.kind == PT_K_COMP)
+    snprintf(buf, n, "k_sweep_comp<%s,%d,%d,%d,%d,trace=%d>", real, pl.nik[0], pl.nik[1], pl.nik[2], pl.nik[3], trace ? 1 : 0);
   else snprintf(buf, n, "k_sweep_group<%s,%d,%d,trace=%d>", real, pl.lanes, pl.ni, trace ? 1 : 0);
 }
 
 cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, uint32_t t0, int n_sweeps,
                             cudaStream_t stream)
 {
-  SweepFn fn = kernel_of(pl, precision, d.tr_move != nullptr);
+  PtSweepFn fn = kernel_of(pl, precision, d.tr_move != nullptr);
   if (!fn) return cudaErrorInvalidValue;
   fn<<<dim3(pl.grid), dim3(pl.threads), pl.smem_bytes, stream>>>(d, pl, t0, n_sweeps);
   return cudaGetLastError();

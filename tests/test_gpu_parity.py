@@ -80,11 +80,12 @@ def test_config4_one_cta_per_replica(lanes):
 
 def test_config5_full_run_all_64_ensembles():
     """The throughput batch exactly as bench.py times it: 64 ensembles x 64 replicas, N=100, 10^3 sweeps,
-    exchange every 10, default mapping (k_sweep_mixed<double,13,10>: 147 CTAs of 28 chains; the last CTA is
-    partly filled -- chains 4088..4095 = the tail of ensemble 63 -- and its inactive lanes clone chain C-1).
+    exchange every 10, default mapping (k_sweep_seven<double,13,10>: 7 chains per SM sub-partition as 4 x 8 + 3 x 10
+    lanes, 147 CTAs of 28 chains; the last CTA is partly filled -- chains 4088..4095 = the tail of ensemble 63 --
+    and its inactive lanes clone chain C-1).
     One oracle run of all 64 ensembles; the GPU runs twice, untraced (the timed kernel) and traced; every
     decision of all 4096 chains is compared."""
-    rep, g, _ = _both(synth.make_inputs(5), 1000, nbins=4096, expect_kernel="k_sweep_mixed<double,13,10,")
+    rep, g, _ = _both(synth.make_inputs(5), 1000, nbins=4096, expect_kernel="k_sweep_seven<double,13,10,")
     info = g[0]["launch_info"]
     assert info["chains_per_cta"] == 28 and info["grid"] == 147
     assert g[0]["counters"] == (1000, 100)
@@ -111,16 +112,37 @@ def test_config5_sampled_ensembles_of_the_full_batch():
 
 def test_mixed_mapping_at_the_papers_chain_length():
     """N = 55, 40 ensembles x 64 replicas = 2560 chains: between 4 and 7 chains per SM sub-partition, so
-    the planner maps 4 chains x 8 lanes + 3 chains x 10 lanes on every one (k_sweep_mixed<7, 6>)."""
+    the planner spreads 18 chains over every SM: sub-partition loads 5, 5, 4, 4 (k_sweep_comp<7,6,4,2>)."""
     N, M, E = 55, 64, 40
     T = synth.temperature_ladder(M, 0.15, 3.0)
     reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T), synth.seeds(3, E, rank=3),
                          synth.random_walk_conformations(E, M, N, seed=5564), 100, 10, label="mixed N=55",
-                         expect_kernel="k_sweep_mixed<double,7,6,")
-    assert runs[False][0]["launch_info"]["chains_per_cta"] == 28
+                         expect_kernel="k_sweep_comp<double,7,6,4,2,")
+    assert runs[False][0]["launch_info"]["chains_per_cta"] == 18
 
 
 # ---- variants and edge cases ----------------------------------------------------------------
+
+# (N, chains) -> chains per CTA and the sub-partition loads the planner must produce on 148 SMs
+COMPOSED = [(30, 600, 5), (55, 4144, 28), (30, 1336, 10), (30, 2000, 14), (30, 2960, 20), (30, 3400, 23), (30, 3848, 26),
+            (30, 4440, 30), (30, 4736, 32), (30, 5000, 17), (17, 1200, 9), (64, 2400, 17), (80, 3000, 21),
+            (104, 1480, 10), (128, 1000, 7), (100, 2376, 17)]
+
+
+@pytest.mark.parametrize("N,C,q", COMPOSED, ids=[f"N{n}_C{c}" for n, c, _ in COMPOSED])
+def test_composed_ctas(N, C, q):
+    """Every composition of k_sweep_comp (SM sub-partition loads 1..8 as warps of 32, 16, 10 and 8 lanes per chain,
+    two waves beyond 4736 chains) and every class of chain lengths around the table's N, both instantiations:
+    chains spread evenly over the SMs, so the time has no staircase in the number of replicas
+    beyond the one of the most loaded sub-partition."""
+    M = 8
+    E = C // M
+    T = synth.temperature_ladder(M, 0.3, 2.5)
+    reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T), synth.seeds(8, E, rank=N),
+                         synth.random_walk_conformations(E, M, N, seed=77000 + N + C), 20, 10, nbins=16,
+                         label=f"composed N={N} C={C}", expect_kernel="k_sweep_seven<double,7,6," if q == 28 else "k_sweep_comp<double,")
+    assert runs[False][0]["launch_info"]["chains_per_cta"] == q
+
 
 def test_random_pick_mode():
     """Paper-literal monomer choice in every mapping family."""
@@ -151,8 +173,8 @@ def _max_abs_energy(conf):
 # (label, N, M, E, lanes, kernel the planner must pick, sweeps, exchange_every)
 OVERLAP_CASES = [
     ("config1_shape", 13, 8, 1, 0, "k_sweep_group<double,16,1,", 150, 10),
-    ("mixed_13_10", 100, 64, 40, 0, "k_sweep_mixed<double,13,10,", 40, 10),
-    ("mixed_7_6", 55, 64, 40, 0, "k_sweep_mixed<double,7,6,", 60, 10),
+    ("comp_13_10_7_4", 100, 64, 40, 0, "k_sweep_comp<double,13,10,7,4,", 40, 10),
+    ("comp_7_6_4_2", 55, 64, 40, 0, "k_sweep_comp<double,7,6,4,2,", 60, 10),
     ("config4_shape", 309, 128, 1, 0, "k_sweep_group<double,32,10,", 40, 20),
     ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
     ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
