@@ -262,8 +262,9 @@ def run_reference(args, rank, world):
     inp = synth.make_inputs(args.config)
     wl = inp.workload
     cores = host_cores()
-    n_ens = min(wl.E, 2)
-    n_sweeps = min(args.sweeps or wl.n_sweeps, max(wl.exchange_every, 100 if wl.N >= 50 else 1000))
+    # about one second of oracle time per step on 16 cores (config 5: 16 ensembles x 200 sweeps = 2e7 moves)
+    n_ens = min(wl.E, 16)
+    n_sweeps = min(args.sweeps or wl.n_sweeps, max(wl.exchange_every, 200 if wl.N >= 50 else 2000))
     for _ in range(args.warmup):
         oracle_sample_run(inp, n_ens, n_sweeps, cores)
     moves, times = oracle_sample_run(inp, n_ens, n_sweeps, cores, reps=args.steps)
@@ -457,13 +458,14 @@ def run_ours(args, rank, world, local):
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = host_cores()
-        ne, ns = min(wl.E, 8), min(n_sweeps, 200 if wl.N >= 50 else 2000)
+        # ~10 s of wall time on 16 cores for config 5 (2e8 moves at ~2e7 moves/s); the small configs whole
+        ne, ns = wl.E, min(n_sweeps, 500 if wl.N >= 50 else 10000)
         moves, times = oracle_sample_run(inp, ne, ns, cores)
         cpu_baseline = {"value": moves / times[0], "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": f"first {ne} of {wl.E} ensembles ({ne * wl.M} chains), {ns} of {n_sweeps} sweeps, "
                                   f"exchange every {S}; {times[0]:.2f} s wall on {cores} threads"}
         # the paper's convention is ONE core: a smaller sample on one thread
-        ns1 = max(S, ns // 4)
+        ns1 = max(S, ns // 2)
         moves1, times1 = oracle_sample_run(inp, 1, ns1, 1)
         cpu_baseline["one_thread"] = {"value": moves1 / times1[0], "unit": UNIT, "cores": 1,
                                       "sample": f"first ensemble ({wl.M} chains), {ns1} sweeps; {times1[0]:.2f} s wall"}

@@ -63,27 +63,25 @@ struct PtLaunch {
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
   int kind;            // PT_K_GROUP, PT_K_COMP or PT_K_CTA
   int stagger;         // PT_K_GROUP: start delay in cycles per rank of a warp on its sub-partition (0 = none)
-  // PT_K_COMP: warps of different kinds in one CTA (k_sweep_comp); kind 0, 1, 2, 3 = 8, 10, 16, 32 lanes per chain
-  int nik[4];          // partner-loop iterations of the four kinds of warp (template arguments of the kernel)
+  // PT_K_COMP / PT_K_SEVEN: warps of different kinds in one CTA; kind 0, 1, 2, 3 = 8, 16, 32, 10 lanes per chain
+  // (k_sweep_comp uses 0..2; k_sweep_seven 0 for warps 0..3 and 3 for warps 4..7)
+  int nik[4];          // partner-loop iterations of each kind of warp (template arguments of the kernel; 0 = unused)
   int kstride[4];      // shared-memory stride between the chains of a warp of each kind, in Reals
   int wkind[8];        // kind of warp w
   int wfirst[8];       // first chain of warp w within the CTA
+  int wcount[8];       // chains of warp w (<= 32 / lanes; the other chain slots stay idle)
   int woff[8];         // shared-memory offset of warp w's first chain, in Reals
   int wdelay[8];       // start delay of warp w in cycles
 };
 
-enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2 };
+enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4 };
 
 // Kernel tables, one per translation unit that instantiates sweep kernels (nullptr = not in this unit).
 PtSweepFn pt_lookup_group(int lanes, int ni, int precision, bool trace);   // pt_sweep_group.cu
 PtSweepFn pt_lookup_cta(int precision, bool trace);                        // pt_sweep_group.cu
-PtSweepFn pt_lookup_comp(const int nik[4], int precision, bool trace);     // pt_sweep_comp*.cu
+PtSweepFn pt_lookup_comp(int kind, const int nik[4], int precision, bool trace);   // pt_sweep_comp*.cu
 // the unrolled variants of k_sweep_group: smallest NI >= ni_needed for this lane count, 0 = run-time loop
 int pt_group_variant(int lanes, int ni_needed);
-// the instantiated (N8, N10, N16, N32) class that covers chain length N with the fewest padded slots; `seven`:
-// the composition is 7 chains on every sub-partition, for which k_sweep_seven (class (N8, N10, -1, -1)) is
-// preferred where it is instantiated for exactly this N; false = no class
-bool pt_comp_class(int N, bool seven, int nik[4]);
 
 
 // pt_sweep.cu

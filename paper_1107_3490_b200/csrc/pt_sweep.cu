@@ -8,33 +8,26 @@
 #include "pt_sweep_classes.h"
 
 // one lookup per translation unit of pt_sweep_classes.h
-#define PT_DECL(u) PtSweepFn pt_lookup_comp_##u(const int nik[4], int precision, bool trace);
+#define PT_DECL(u) PtSweepFn pt_lookup_comp_##u(int kind, const int nik[4], int precision, bool trace);
 PT_DECL(0) PT_DECL(1) PT_DECL(2) PT_DECL(3) PT_DECL(4) PT_DECL(5) PT_DECL(6) PT_DECL(7)
 #undef PT_DECL
 static_assert(PT_COMP_UNITS == 8, "declare and call the lookup of every unit");
 
-PtSweepFn pt_lookup_comp(const int nik[4], int precision, bool trace)
+PtSweepFn pt_lookup_comp(int kind, const int nik[4], int precision, bool trace)
 {
-  PtSweepFn (*const units[])(const int*, int, bool) = {pt_lookup_comp_0, pt_lookup_comp_1, pt_lookup_comp_2,
-                                                       pt_lookup_comp_3, pt_lookup_comp_4, pt_lookup_comp_5,
-                                                       pt_lookup_comp_6, pt_lookup_comp_7};
+  PtSweepFn (*const units[])(int, const int*, int, bool) = {pt_lookup_comp_0, pt_lookup_comp_1, pt_lookup_comp_2,
+                                                            pt_lookup_comp_3, pt_lookup_comp_4, pt_lookup_comp_5,
+                                                            pt_lookup_comp_6, pt_lookup_comp_7};
   for (auto f : units)
-    if (PtSweepFn k = f(nik, precision, trace)) return k;
+    if (PtSweepFn k = f(kind, nik, precision, trace)) return k;
   return nullptr;
 }
 
 namespace {
 
-struct CompClass { int nik[4]; };
-#define PT_COMP(A, B, C, D) {{A, B, C, D}},
-#define PT_SEVEN(A, B) {{A, B, -1, -1}},
-const CompClass kCompClasses[] = {PT_COMP_CLASSES_0 PT_COMP_CLASSES_1 PT_COMP_CLASSES_2 PT_COMP_CLASSES_3
-                                  PT_COMP_CLASSES_4 PT_COMP_CLASSES_5 PT_COMP_CLASSES_6 PT_COMP_CLASSES_7};
-#undef PT_COMP
-#undef PT_SEVEN
-
-const int kLanesOfKind[4] = {8, 10, 16, 32};
-const int kChainsOfKind[4] = {4, 3, 2, 1};
+// kinds of warp: lanes per chain and chain slots per warp
+const int kLanesOfKind[4] = {8, 16, 32, 10};
+const int kSlotsOfKind[4] = {4, 2, 1, 3};
 
 int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
@@ -56,76 +49,98 @@ int stagger_cycles(int ni) { return (int)(2.1 * (26.0 * ni + 70.0)); }
 PtSweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return pt_lookup_cta(precision, trace);
-  if (pl.kind == PT_K_COMP) return pt_lookup_comp(pl.nik, precision, trace);
+  if (pl.kind == PT_K_COMP || pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
+    return pt_lookup_comp(pl.kind, pl.nik, precision, trace);
   return pt_lookup_group(pl.lanes, pl.ni, precision, trace);
 }
 
-// Composed CTAs (k_sweep_comp): chains spread evenly over the SMs, one CTA per SM and wave, every sub-partition
-// one or two warps chosen for its load.  Returns false if this shape is not covered.
-bool plan_comp(const PtDev& d, int real_bytes, int sms, PtLaunch* out)
+struct WarpSpec { int kind, count; };   // kind < 0: no warp
+
+// k_sweep_comp: the (at most) two warps of a sub-partition that holds `load` chains; a second candidate for
+// three chains (2 x 16 + 1 x 32 lanes instead of 3 of 4 x 8), chosen by the cost model below
+const WarpSpec kCompWarps[9][2] = {{{-1, 0}, {-1, 0}}, {{2, 1}, {-1, 0}}, {{1, 2}, {-1, 0}}, {{0, 3}, {-1, 0}},
+                                   {{0, 4}, {-1, 0}},  {{0, 4}, {2, 1}},  {{0, 4}, {1, 2}},  {{0, 4}, {0, 3}},
+                                   {{0, 4}, {0, 4}}};
+const WarpSpec kThreeAlt[2] = {{1, 2}, {2, 1}};
+
+// Cost model of one sub-partition, in cycles per step (fit to profiles/r02_paper_timing.md): a warp issues about
+// 60 slots per partner iteration (26 fp64 instructions that take the fp64 pipe for two cycles each, 10 others) and
+// 280 for the serial part of the step; one warp alone on a sub-partition is latency-bound (x 1.35), two warps share
+// the issue port (x 1.08 of the sum).
+double warp_issue(int ni) { return 60.0 * ni + 280.0; }
+double subpartition_cost(const WarpSpec w[2], const int nik[4])
 {
+  if (w[0].kind < 0) return 0.0;
+  if (w[1].kind < 0 || w[1].count == 0) return 1.35 * warp_issue(nik[w[0].kind]);
+  return 1.08 * (warp_issue(nik[w[0].kind]) + warp_issue(nik[w[1].kind]));
+}
+
+const WarpSpec* comp_warps(int load, const int nik[4])
+{
+  if (load == 3 && subpartition_cost(kThreeAlt, nik) < subpartition_cost(kCompWarps[3], nik)) return kThreeAlt;
+  return kCompWarps[load];
+}
+
+// Composed CTAs (k_sweep_comp, k_sweep_seven): chains spread evenly over the SMs, one CTA per SM and wave, every
+// sub-partition one or two warps chosen for its load.  Returns false if this shape is not covered.
+bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch* out)
+{
+  if (d.N < 17 || d.N > 128) return false;
   PtLaunch pl{};
   const long long cap = 32ll * sms;                       // 8 chains per sub-partition: two warps of 4
   const long long waves = (d.C + cap - 1) / cap;
   const int q = (int)((d.C + sms * waves - 1) / (sms * waves));   // chains per CTA
-  // kinds of the (at most) two warps of a sub-partition that holds `load` chains; -1 = no warp
-  static const int kWarps[9][2] = {{-1, -1}, {3, -1}, {2, -1}, {1, -1}, {0, -1}, {1, 2}, {1, 1}, {0, 1}, {0, 0}};
-  if (!pt_comp_class(d.N, q == 28, pl.nik)) return false;
+  const int nc = (d.N + 7) / 8;
+  pl.nik[0] = nc; pl.nik[1] = (nc + 1) / 2; pl.nik[2] = (nc + 3) / 4; pl.nik[3] = (d.N + 9) / 10;
   pl.kind = PT_K_COMP;
+  // the seven-chain layout (4 x 8 + up to 3 x 10 lanes) where it is instantiated for this N and predicted faster
+  if (q > 16 && q <= 28) {
+    PtLaunch probe = pl;
+    probe.kind = PT_K_SEVEN;
+    if (kernel_of(probe, precision, false)) {
+      double cost_comp = 0.0, cost_seven = 0.0;
+      for (int sp = 0; sp < 4; ++sp) {
+        const int load = q / 4 + (sp < q % 4 ? 1 : 0);
+        const WarpSpec sv[2] = {{0, load < 4 ? load : 4}, {load > 4 ? 3 : -1, load > 4 ? load - 4 : 0}};
+        const double a = subpartition_cost(comp_warps(load, pl.nik), pl.nik), b = subpartition_cost(sv, pl.nik);
+        if (a > cost_comp) cost_comp = a;
+        if (b > cost_seven) cost_seven = b;
+      }
+      if (cost_seven < cost_comp) pl.kind = q == 28 ? PT_K_SEVEN_FULL : PT_K_SEVEN;
+    }
+  }
   pl.chains_per_cta = q;
   pl.grid = (int)((d.C + q - 1) / q);
-  for (int k = 0; k < 4; ++k)
-    pl.kstride[k] = pl.nik[k] > 0 ? chain_stride(kLanesOfKind[k] * pl.nik[k], kLanesOfKind[k], real_bytes) : 0;
+  for (int k = 0; k < 4; ++k) pl.kstride[k] = chain_stride(kLanesOfKind[k] * pl.nik[k], kLanesOfKind[k], real_bytes);
   int first = 0, off = 0, nwarps = 4, lanes_min = 32;
   for (int w = 0; w < 8; ++w) {
-    const int sp = w & 3, load = q / 4 + (sp < q % 4 ? 1 : 0);
-    const int k = kWarps[load][w >> 2];
-    if (k < 0) {
-      pl.wkind[w] = 3;
-      pl.wfirst[w] = 1 << 30;        // beyond every chain: the warp leaves at once
-      continue;
-    }
-    if (w >= 4) nwarps = 8;
-    pl.wkind[w] = k;
+    const int sp = w & 3, load = q / 4 + (sp < q % 4 ? 1 : 0), r = w >> 2;
+    WarpSpec ws = comp_warps(load, pl.nik)[r];
+    if (pl.kind != PT_K_COMP) ws = r == 0 ? WarpSpec{0, load < 4 ? load : 4} : WarpSpec{3, load > 4 ? load - 4 : 0};
+    pl.wkind[w] = ws.kind < 0 ? 2 : ws.kind;
     pl.wfirst[w] = first;
+    pl.wcount[w] = ws.kind < 0 ? 0 : ws.count;
     pl.woff[w] = off;
-    pl.wdelay[w] = (w >= 4 && kWarps[load][0] == k) ? stagger_cycles(pl.nik[k]) : 0;
-    first += kChainsOfKind[k];
-    off += kChainsOfKind[k] * pl.kstride[k];
-    if (kLanesOfKind[k] < lanes_min) lanes_min = kLanesOfKind[k];
+    if (ws.kind < 0 || ws.count == 0) continue;
+    if (r == 1) nwarps = 8;
+    pl.wdelay[w] = (r == 1 && comp_warps(load, pl.nik)[0].kind == ws.kind && pl.kind == PT_K_COMP) ? stagger_cycles(pl.nik[ws.kind]) : 0;
+    first += ws.count;
+    off += kSlotsOfKind[ws.kind] * pl.kstride[ws.kind];
+    if (kLanesOfKind[ws.kind] < lanes_min) lanes_min = kLanesOfKind[ws.kind];
   }
   if (first != q) return false;
+  if (pl.kind != PT_K_COMP) nwarps = 8;
   pl.lanes = lanes_min;
   pl.ni = pl.nik[0];
   pl.Ns = 8 * pl.nik[0];
   pl.threads = 32 * nwarps;
   pl.smem_bytes = off * real_bytes;
+  if (!kernel_of(pl, precision, false)) return false;
   *out = pl;
   return true;
 }
 
 }  // namespace
-
-bool pt_comp_class(int N, bool seven, int nik[4])
-{
-  if (N < 17) return false;
-  const CompClass* best = nullptr;
-  int best_waste = 0;
-  for (const CompClass& c : kCompClasses) {
-    const bool is_seven = c.nik[2] < 0;      // k_sweep_seven: exact fit only, and only for that composition
-    bool ok = is_seven ? seven : true;
-    int waste = is_seven ? -1 : 0;
-    for (int k = 0; k < (is_seven ? 2 : 4); ++k) {
-      const int need = (N + kLanesOfKind[k] - 1) / kLanesOfKind[k];
-      ok = ok && (is_seven ? c.nik[k] == need : c.nik[k] >= need);
-      waste += c.nik[k] - need;
-    }
-    if (ok && (!best || waste < best_waste)) { best = &c; best_waste = waste; }
-  }
-  if (!best) return false;
-  for (int k = 0; k < 4; ++k) nik[k] = best->nik[k];
-  return true;
-}
 
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan)
 {
@@ -146,7 +161,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   if (L == 0) {
     // More chains than SM sub-partitions: composed CTAs, chains spread evenly over the SMs (no staircase in
     // the number of replicas beyond the one of the most loaded sub-partition).
-    if ((long long)d.C > smsp) done = plan_comp(d, real_bytes, sms, &pl);
+    if ((long long)d.C > smsp) done = plan_comp(d, precision, real_bytes, sms, &pl);
     if (!done) {
       // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
       // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
@@ -214,10 +229,11 @@ void pt_sweep_kernel_desc(const PtLaunch& pl, int precision, bool trace, char* b
 {
   const char* real = precision == PT_F32 ? "float" : "double";
   if (pl.kind == PT_K_CTA) snprintf(buf, n, "k_sweep_cta<%s,threads=%d,trace=%d>", real, pl.threads, trace ? 1 : 0);
-  else if (pl.kind == PT_K_COMP && pl.nik[2] < 0)
-    snprintf(buf, n, "k_sweep_seven<%s,%d,%d,trace=%d>", real, pl.nik[0], pl.nik[1], trace ? 1 : 0);
+  else if (pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
+    snprintf(buf, n, "k_sweep_seven<%s,%d,%d,%s,trace=%d>", real, pl.nik[0], pl.nik[3],
+             pl.kind == PT_K_SEVEN_FULL ? "full" : "partial", trace ? 1 : 0);
   else if (pl.kind == PT_K_COMP)
-    snprintf(buf, n, "k_sweep_comp<%s,%d,%d,%d,%d,trace=%d>", real, pl.nik[0], pl.nik[1], pl.nik[2], pl.nik[3], trace ? 1 : 0);
+    snprintf(buf, n, "k_sweep_comp<%s,%d,%d,%d,trace=%d>", real, pl.nik[0], pl.nik[1], pl.nik[2], trace ? 1 : 0);
   else snprintf(buf, n, "k_sweep_group<%s,%d,%d,trace=%d>", real, pl.lanes, pl.ni, trace ? 1 : 0);
 }
 

@@ -41,9 +41,10 @@ struct ChainCtx {
   unsigned acc, brej;
 };
 
-__device__ __forceinline__ void ctx_load(const PtDev& d, int s, ChainCtx& c)
+// `end`: first chain this warp (or CTA) must NOT touch; chains at or beyond it are inactive clones of chain C-1
+__device__ __forceinline__ void ctx_load(const PtDev& d, int s, int end, ChainCtx& c)
 {
-  c.active = s < d.C;
+  c.active = s < end;   // callers pass end <= d.C
   c.s = c.active ? s : d.C - 1;
   c.e = c.s / d.M;
   c.i = d.temp_of_slot[c.s];

@@ -306,12 +306,12 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
 // NI > 0: the partner loop has exactly NI iterations (Ns = NI * L) and is unrolled completely, so
 // that the serial stream of a step (bond sqrt / log, log u) sits in the same basic block as the
 // pair terms and the scheduler overlaps the two.  NI = 0: run-time trip count Ns / L.
-// One warp's share of a sweep launch: G = 32 / L chains starting at slot `chain0`, coordinates at
+// One warp's share of a sweep launch: up to G = 32 / L chains, slots `chain0` .. `chain_end` - 1, coordinates at
 // `smem0` (stride `sstride` Reals between chains, Ns slots per coordinate array).  `delay`: cycles to
 // wait before the first step (phase stagger).
 template <typename Real, int L, int NI, bool TRACE>
-__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns, int chain0, int delay,
-                                           const uint32_t t0, const int n_sweeps)
+__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns, int chain0, int chain_end,
+                                           int delay, const uint32_t t0, const int n_sweeps)
 {
   static_assert(L >= 8 && L <= 32, "lanes per chain");
   constexpr int G = 32 / L;
@@ -327,7 +327,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
   const int N = d.N;
 
   ChainCtx c;
-  ctx_load(d, chain0 + g, c);
+  ctx_load(d, chain0 + g, chain_end, c);
   const Real width = (Real)d.width[c.i];
   const PtLJ<Real> lj(d);
 
@@ -465,21 +465,19 @@ __global__ void __launch_bounds__(256, 1) k_sweep_group(const PtDev d, const PtL
   constexpr int G = 32 / L;
   const int warp = threadIdx.x >> 5;
   sweep_warp<Real, L, NI, TRACE>(d, reinterpret_cast<Real*>(smem_raw) + (size_t)(warp * G) * pl.sstride, pl.sstride, pl.Ns,
-                                 blockIdx.x * pl.chains_per_cta + warp * G, pl.stagger * (warp >> 2), t0, n_sweeps);
+                                 blockIdx.x * pl.chains_per_cta + warp * G, d.C, pl.stagger * (warp >> 2), t0, n_sweeps);
 }
 
 // Composed CTA against wave quantisation (the paper's staircase).  With uniform warps a
 // sub-partition jumps from one warp to two as soon as the chains per SM pass a multiple of 4, 8 or 16, and the
 // most loaded sub-partition sets the time.  Here the chains are spread evenly over the SMs (q = ceil(C / #SM) per
-// CTA, one CTA per SM), and every sub-partition gets one or two warps whose kinds are chosen for its load:
-//   1 chain: 32 lanes   2: 2 x 16   3: 3 x 10   4: 4 x 8   5: 3 x 10 + 2 x 16   6: 3 x 10 + 3 x 10
-//   7: 4 x 8 + 3 x 10   8: 4 x 8 + 4 x 8
-// (lanes 30, 31 of a 10-lane warp idle).  Warp w of a CTA runs on sub-partition w mod 4.  N8, N10, N16, N32 =
-// partner iterations of the four kinds of warp (L x NI slots >= N; 0 = this kind is not compiled in: with fewer
-// code paths ptxas allocates the remaining ones better, measured 3.5 % on the throughput batch).  The throughput
-// batch (4096 chains, N = 100) is 7 chains per sub-partition: 4 x 8 lanes (13 iterations) + 3 x 10 lanes (10
-// iterations), 28 chains per CTA: k_sweep_comp<double, 13, 10, 0, 0>.
-template <typename Real, int N8, int N10, int N16, int N32, bool TRACE>
+// CTA, one CTA per SM and wave), and every sub-partition gets one or two warps whose kinds are chosen for its load:
+//   1 chain: 32 lanes   2: 2 x 16   3: 3 of 4 x 8   4: 4 x 8   5: 4 x 8 + 1 x 32   6: 4 x 8 + 2 x 16
+//   7: 4 x 8 + 3 of 4 x 8   8: 4 x 8 + 4 x 8
+// ("3 of 4 x 8": an 8-lane warp with one chain slot left idle).  Warp w of a CTA runs on sub-partition w mod 4; its
+// kind, first chain, number of chains and shared-memory offset come from the launch descriptor.  N8, N16, N32 =
+// partner iterations of the three kinds of warp (L x NI slots >= N).
+template <typename Real, int N8, int N16, int N32, bool TRACE>
 __global__ void __launch_bounds__(256, 1) k_sweep_comp(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                     const int n_sweeps)
 {
@@ -487,40 +485,50 @@ __global__ void __launch_bounds__(256, 1) k_sweep_comp(const PtDev d, const PtLa
   const int warp = threadIdx.x >> 5;
   const int kind = pl.wkind[warp];
   const int chain0 = blockIdx.x * pl.chains_per_cta + pl.wfirst[warp];
-  if (chain0 >= d.C) return;                 // a partly filled last CTA: warps without any chain
+  const int chain_end = min(chain0 + pl.wcount[warp], (int)min((long long)d.C, (long long)(blockIdx.x + 1) * pl.chains_per_cta));
+  if (chain0 >= chain_end) return;           // no chain for this warp (a partly filled last CTA, an unused warp slot)
   Real* base = reinterpret_cast<Real*>(smem_raw) + pl.woff[warp];
   const int delay = pl.wdelay[warp];
-  // a kind with 0 iterations is not part of this instantiation (the planner never asks for it)
-  if constexpr (N8 > 0)
-    if (kind == 0) sweep_warp<Real, 8, N8, TRACE>(d, base, pl.kstride[0], 8 * N8, chain0, delay, t0, n_sweeps);
-  if constexpr (N10 > 0)
-    if (kind == 1) sweep_warp<Real, 10, N10, TRACE>(d, base, pl.kstride[1], 10 * N10, chain0, delay, t0, n_sweeps);
-  if constexpr (N16 > 0)
-    if (kind == 2) sweep_warp<Real, 16, N16, TRACE>(d, base, pl.kstride[2], 16 * N16, chain0, delay, t0, n_sweeps);
-  if constexpr (N32 > 0)
-    if (kind == 3) sweep_warp<Real, 32, N32, TRACE>(d, base, pl.kstride[3], 32 * N32, chain0, delay, t0, n_sweeps);
+  if (kind == 0) sweep_warp<Real, 8, N8, TRACE>(d, base, pl.kstride[0], 8 * N8, chain0, chain_end, delay, t0, n_sweeps);
+  else if (kind == 1) sweep_warp<Real, 16, N16, TRACE>(d, base, pl.kstride[1], 16 * N16, chain0, chain_end, delay, t0, n_sweeps);
+  else sweep_warp<Real, 32, N32, TRACE>(d, base, pl.kstride[2], 32 * N32, chain0, chain_end, delay, t0, n_sweeps);
 }
 
-// The composition "7 chains on every sub-partition" (4 x 8 + 3 x 10 lanes, 28 chains per CTA) with the kinds of the
-// warps fixed at compile time: the mapping of the throughput batch (4096 chains, N = 100).  Same body as
-// k_sweep_comp; ptxas schedules this form 3.5 % better than the four-kind kernel (measured, config 5: 2108 against
-// 2183 cycles per step), so the planner uses it whenever every sub-partition holds exactly 7 chains.  The start
-// delay of the 10-lane warps is passed as a run-time value (always 0): with a literal 0 the wait loop disappears
-// from the code and the schedule ptxas then finds for the step loop is 6 % slower (2246 cycles, measured twice).
-template <typename Real, int N8, int N10, bool TRACE>
+// Seven chains per sub-partition as 4 x 8 lanes + 3 x 10 lanes (lanes 30, 31 of a 10-lane warp idle): the mapping of
+// the throughput batch (4096 chains on 148 SMs, N = 100: 13 and 10 partner iterations, 104 and 100 slots).  A
+// 10-lane warp pays where 10 ceil(N/10) is much closer to N than 8 ceil(N/8) (measured: N = 100 2077 against 2440
+// cycles per step of 4 x 8 + 4 x 8; N = 55 and 64 no gain).  Warps 0..3 are the 8-lane warps, 4..7 the 10-lane ones;
+// the chain counts per warp come from the launch descriptor (6 chains on a sub-partition: 4 + 2).
+// The start delay of the 10-lane warps is passed as a run-time value (always 0): with a literal 0 the wait loop
+// disappears from the code and the schedule ptxas then finds for the step loop is 6 % slower (measured twice).
+// FULL: every sub-partition holds exactly 7 chains (28 per CTA) and the layout is fixed at compile time; otherwise
+// first chain, number of chains and shared-memory offset of every warp come from the launch descriptor.  Same
+// arithmetic; the fixed form is the one ptxas schedules best (measured, config 5: 2108 against 2232 cycles per step).
+template <typename Real, int N8, int N10, bool TRACE, bool FULL>
 __global__ void __launch_bounds__(256, 1) k_sweep_seven(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                      const int n_sweeps)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Real* base = reinterpret_cast<Real*>(smem_raw);
   const int warp = threadIdx.x >> 5;
-  const int cta0 = blockIdx.x * 28;
-  if (warp < 4)
-    sweep_warp<Real, 8, N8, TRACE>(d, base + (size_t)(warp * 4) * pl.kstride[0], pl.kstride[0], 8 * N8, cta0 + warp * 4, 0,
-                                   t0, n_sweeps);
-  else
-    sweep_warp<Real, 10, N10, TRACE>(d, base + (size_t)16 * pl.kstride[0] + (size_t)((warp - 4) * 3) * pl.kstride[1],
-                                     pl.kstride[1], 10 * N10, cta0 + 16 + (warp - 4) * 3, pl.stagger, t0, n_sweeps);
+  if (FULL) {
+    const int cta0 = blockIdx.x * 28;
+    if (warp < 4)
+      sweep_warp<Real, 8, N8, TRACE>(d, base + (size_t)(warp * 4) * pl.kstride[0], pl.kstride[0], 8 * N8, cta0 + warp * 4,
+                                     d.C, 0, t0, n_sweeps);
+    else
+      sweep_warp<Real, 10, N10, TRACE>(d, base + (size_t)16 * pl.kstride[0] + (size_t)((warp - 4) * 3) * pl.kstride[3],
+                                       pl.kstride[3], 10 * N10, cta0 + 16 + (warp - 4) * 3, d.C, pl.stagger, t0, n_sweeps);
+  } else {
+    const int chain0 = blockIdx.x * pl.chains_per_cta + pl.wfirst[warp];
+    const int chain_end = min(chain0 + pl.wcount[warp], (int)min((long long)d.C, (long long)(blockIdx.x + 1) * pl.chains_per_cta));
+    if (chain0 >= chain_end) return;           // no chain for this warp
+    if (warp < 4)
+      sweep_warp<Real, 8, N8, TRACE>(d, base + pl.woff[warp], pl.kstride[0], 8 * N8, chain0, chain_end, 0, t0, n_sweeps);
+    else
+      sweep_warp<Real, 10, N10, TRACE>(d, base + pl.woff[warp], pl.kstride[3], 10 * N10, chain0, chain_end, pl.stagger, t0,
+                                       n_sweeps);
+  }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -538,7 +546,7 @@ __global__ void __launch_bounds__(256, 1) k_sweep_cta(const PtDev d, const PtLau
   const int N = d.N, Ns = pl.Ns;
 
   ChainCtx c;
-  ctx_load(d, blockIdx.x, c);
+  ctx_load(d, blockIdx.x, d.C, c);
   const Real width = (Real)d.width[c.i];
   const PtLJ<Real> lj(d);
 

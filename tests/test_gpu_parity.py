@@ -112,12 +112,12 @@ def test_config5_sampled_ensembles_of_the_full_batch():
 
 def test_mixed_mapping_at_the_papers_chain_length():
     """N = 55, 40 ensembles x 64 replicas = 2560 chains: between 4 and 7 chains per SM sub-partition, so
-    the planner spreads 18 chains over every SM: sub-partition loads 5, 5, 4, 4 (k_sweep_comp<7,6,4,2>)."""
+    the planner spreads 18 chains over every SM: sub-partition loads 5, 5, 4, 4 (k_sweep_comp<7,4,2>)."""
     N, M, E = 55, 64, 40
     T = synth.temperature_ladder(M, 0.15, 3.0)
     reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T), synth.seeds(3, E, rank=3),
                          synth.random_walk_conformations(E, M, N, seed=5564), 100, 10, label="mixed N=55",
-                         expect_kernel="k_sweep_comp<double,7,6,4,2,")
+                         expect_kernel="k_sweep_comp<double,7,4,2,")
     assert runs[False][0]["launch_info"]["chains_per_cta"] == 18
 
 
@@ -131,8 +131,9 @@ COMPOSED = [(30, 600, 5), (55, 4144, 28), (30, 1336, 10), (30, 2000, 14), (30, 2
 
 @pytest.mark.parametrize("N,C,q", COMPOSED, ids=[f"N{n}_C{c}" for n, c, _ in COMPOSED])
 def test_composed_ctas(N, C, q):
-    """Every composition of k_sweep_comp (SM sub-partition loads 1..8 as warps of 32, 16, 10 and 8 lanes per chain,
-    two waves beyond 4736 chains) and every class of chain lengths around the table's N, both instantiations:
+    """Every composition of k_sweep_comp (SM sub-partition loads 1..8 as warps of 32, 16 and 8 lanes per chain, some
+    with an idle chain slot; two waves beyond 4736 chains) and of k_sweep_seven, chain lengths around the table's N,
+    both instantiations:
     chains spread evenly over the SMs, so the time has no staircase in the number of replicas
     beyond the one of the most loaded sub-partition."""
     M = 8
@@ -173,8 +174,9 @@ def _max_abs_energy(conf):
 # (label, N, M, E, lanes, kernel the planner must pick, sweeps, exchange_every)
 OVERLAP_CASES = [
     ("config1_shape", 13, 8, 1, 0, "k_sweep_group<double,16,1,", 150, 10),
-    ("comp_13_10_7_4", 100, 64, 40, 0, "k_sweep_comp<double,13,10,7,4,", 40, 10),
-    ("comp_7_6_4_2", 55, 64, 40, 0, "k_sweep_comp<double,7,6,4,2,", 60, 10),
+    ("comp_13_7_4", 100, 64, 40, 0, "k_sweep_comp<double,13,7,4,", 40, 10),
+    ("comp_7_4_2", 55, 64, 40, 0, "k_sweep_comp<double,7,4,2,", 60, 10),
+    ("seven_13_10_partly_filled", 100, 64, 60, 0, "k_sweep_seven<double,13,10,", 30, 10),
     ("config4_shape", 309, 128, 1, 0, "k_sweep_group<double,32,10,", 40, 20),
     ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
     ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
