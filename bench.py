@@ -408,7 +408,10 @@ def run_ours(args, rank, world, local):
     kernel_name = sim.pt_sweep_kernel_name()
     rec = recorded_ncu(args.precision, args.config, args.lanes)
     rm = rec["metrics"] if rec else {}
-    traffic = (rm.get("dram__bytes_read.sum", 0.0) + rm.get("dram__bytes_write.sum", 0.0)) if rec else None
+    ru = rec.get("units", {}) if rec else {}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1.0, "us": 1e3, "ms": 1e6, "s": 1e9}
+    in_base = lambda k: rm.get(k, 0.0) * scale.get(ru.get(k, ""), 1.0)
+    traffic = (in_base("dram__bytes_read.sum") + in_base("dram__bytes_write.sum")) if rec else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "kernel": kernel_name, "kernel_ms": k_s * 1e3,
                 "peak_kind": f"measured {'fp32' if f32 else 'fp64'} FMA chain (pt_fma_peak), this run",
@@ -421,7 +424,7 @@ def run_ours(args, rank, world, local):
                     "kernel": rec.get("kernel"), "csrc_hash": rec.get("csrc_hash"),
                     "pipe_pct": rm.get("sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active" if f32 else
                                        "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"),
-                    "duration_ns": rm.get("gpu__time_duration.sum"),
+                    "duration_ns": in_base("gpu__time_duration.sum"),
                     "dram_bytes": traffic, "file": str(NCU_RECORD.relative_to(ROOT))}}
 
     # end to end through the C ABI with HOST buffers: pt_init (H2D) + pt_run + pt_read (D2H)
