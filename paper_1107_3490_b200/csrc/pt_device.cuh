@@ -227,6 +227,44 @@ template <typename Real> struct PtVec2;
 template <> struct PtVec2<double> { typedef double2 type; };
 template <> struct PtVec2<float> { typedef float2 type; };
 
+// ---- packed fp32 pairs (sm_100a: add / mul / fma on two floats in one 64-bit register pair, SASS FADD2 / FMUL2 /
+// FFMA2): the fp32 sweep kernels do the arithmetic of two adjacent partners with one instruction.
+typedef unsigned long long PtF2;
+__device__ __forceinline__ PtF2 pt_f2(float lo, float hi)
+{
+  PtF2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void pt_f2_split(PtF2 v, float& lo, float& hi)
+{
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ PtF2 pt_add2(PtF2 a, PtF2 b)
+{
+  PtF2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ PtF2 pt_sub2(PtF2 a, PtF2 b)
+{
+  PtF2 r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ PtF2 pt_mul2(PtF2 a, PtF2 b)
+{
+  PtF2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ PtF2 pt_fma2(PtF2 a, PtF2 b, PtF2 c)
+{
+  PtF2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
 // One chain's coordinates in shared memory: (x, y) pairs in one array, z in another, so that a
 // partner costs one 128-bit and one 64-bit load (fp64) with consecutive lanes on consecutive banks.
 template <typename Real> struct PtCoords {
@@ -247,5 +285,20 @@ template <typename Real> struct PtCoords {
     v.x = x; v.y = y;
     xy[j] = v;
     z[j] = zz;
+  }
+};
+
+// fp32: three separate arrays x[], y[], z[], so that the coordinates of two adjacent monomers 2p, 2p+1 are one
+// 64-bit load per component and arrive as packed pairs (get2).
+template <> struct PtCoords<float> {
+  float *x, *y, *z;
+  __device__ __forceinline__ PtCoords(float* base, int slots) : x(base), y(base + slots), z(base + 2 * (size_t)slots) {}
+  __device__ __forceinline__ void get(int j, float& xx, float& yy, float& zz) const { xx = x[j]; yy = y[j]; zz = z[j]; }
+  __device__ __forceinline__ void set(int j, float xx, float yy, float zz) const { x[j] = xx; y[j] = yy; z[j] = zz; }
+  __device__ __forceinline__ void get2(int p, PtF2& xx, PtF2& yy, PtF2& zz) const
+  {
+    xx = reinterpret_cast<const PtF2*>(x)[p];
+    yy = reinterpret_cast<const PtF2*>(y)[p];
+    zz = reinterpret_cast<const PtF2*>(z)[p];
   }
 };

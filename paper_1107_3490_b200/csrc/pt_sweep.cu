@@ -38,10 +38,17 @@ constexpr int kSmemCap = 200 * 1024;   // dynamic shared memory any sweep kernel
 int chain_stride(int Ns, int L, int real_bytes)
 {
   const int Q = 128 / real_bytes;
+  // fp32 unrolled kernels read 8-byte pairs: two groups of 8 (10) lanes share a 128-byte phase when the second
+  // starts 64 (80) bytes after the first
+  const int want = real_bytes == 4 ? (L == 8 ? 16 : (L == 10 ? 20 : L % Q)) : L % Q;
   int ss = 3 * Ns;
-  while (ss % Q != L % Q) ++ss;
+  while (ss % Q != want) ++ss;
   return ss;
 }
+
+// table slots per coordinate array of an unrolled kernel: L lanes x ni iterations; the fp32 kernels take two partners
+// per lane and iteration (pair_group_f2), i.e. an even number of iterations
+int table_slots(int L, int ni, int real_bytes) { return real_bytes == 4 ? 2 * L * ((ni + 1) / 2) : L * ni; }
 
 // phase stagger between two warps of the same kind on one sub-partition: about the fp64 time of one partner loop
 int stagger_cycles(int ni) { return (int)(2.1 * (26.0 * ni + 70.0)); }
@@ -111,7 +118,8 @@ bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch*
   }
   pl.chains_per_cta = q;
   pl.grid = (int)((d.C + q - 1) / q);
-  for (int k = 0; k < 4; ++k) pl.kstride[k] = chain_stride(kLanesOfKind[k] * pl.nik[k], kLanesOfKind[k], real_bytes);
+  for (int k = 0; k < 4; ++k)
+    pl.kstride[k] = chain_stride(table_slots(kLanesOfKind[k], pl.nik[k], real_bytes), kLanesOfKind[k], real_bytes);
   int first = 0, off = 0, nwarps = 4, lanes_min = 32;
   for (int w = 0; w < 8; ++w) {
     const int sp = w & 3, load = q / 4 + (sp < q % 4 ? 1 : 0), r = w >> 2;
@@ -184,7 +192,7 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     pl.lanes = L;
     pl.kind = PT_K_GROUP;
     pl.ni = ni;
-    pl.Ns = ni > 0 ? ni * L : round_up(d.N, L);
+    pl.Ns = ni > 0 ? table_slots(L, ni, real_bytes) : round_up(d.N, L);
     pl.sstride = chain_stride(pl.Ns, L, real_bytes);
     // one CTA per SM when there are enough warps (its warps are dealt round-robin to the four
     // sub-partitions, so they are balanced by construction); single-warp CTAs otherwise

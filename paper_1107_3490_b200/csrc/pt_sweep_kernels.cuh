@@ -300,6 +300,118 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
   return fma(lj.A, (acc[0] + acc[1]) + (acc[2] + acc[3]), -lj.C * (Real)cnt);
 }
 
+#ifndef PT_F32_ONE_RCP
+#define PT_F32_ONE_RCP 1
+#endif
+// ---- fp32: two adjacent partners per lane and iteration, packed arithmetic --------------------------------
+// The fp32 kernels are bound by issue slots, not by a pipe (ncu: 70 % of the issue slots, 40 % of the FMA pipe), so
+// they do the arithmetic of the partners 2p and 2p+1 with one FADD2 / FMUL2 / FFMA2 each: iteration `it` of lane `lig`
+// takes the pair p = lig + L it (three 64-bit loads from the x[], y[], z[] arrays).  The cutoff is applied as Eq. (1)
+// prints it, E_LJ(min(r, r_c)) - E_LJ(r_c): r^2 is clamped to r_c^2 (one FMNMX), a pair beyond the cutoff then has
+// u = u_c in the old and in the new position and (v_n - v_o)(v_n + v_o) is exactly 0 -- no mask, no count of inside
+// pairs, and C drops out.  The moved monomer itself gets r^2 = r_c^2 in both positions.  (The fp64 path cannot clamp:
+// it has no single-instruction 64-bit minimum.)  The fp32 path is checked statistically (tests/test_gpu_fp32_stat.py).
+template <int L, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
+__device__ __forceinline__ void pair_group_f2(const PtLJ<float>& lj, const PtCoords<float>& X, int p0, int m, PtF2 xo2,
+                                              PtF2 yo2, PtF2 zo2, PtF2 tdx2, PtF2 tdy2, PtF2 tdz2, PtF2 dd2, PtF2 mhc2,
+                                              PtF2 (&acc)[2], BondChain<float>& side)
+{
+#define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
+  PtF2 bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) X.get2(p0 + (BEGIN + u) * L, bx[u], by[u], bz[u]);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) { bx[u] = pt_sub2(xo2, bx[u]); by[u] = pt_sub2(yo2, by[u]); bz[u] = pt_sub2(zo2, bz[u]); }
+  PT_SIDE(0);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = pt_mul2(bx[u], bx[u]);
+  PT_SIDE(1);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = pt_fma2(by[u], by[u], ro[u]);
+  PT_SIDE(2);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) ro[u] = pt_fma2(bz[u], bz[u], ro[u]);
+  PT_SIDE(3);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = pt_add2(ro[u], dd2);
+  PT_SIDE(4);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = pt_fma2(tdz2, bz[u], rn[u]);
+  PT_SIDE(5);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = pt_fma2(tdy2, by[u], rn[u]);
+  PT_SIDE(6);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) rn[u] = pt_fma2(tdx2, bx[u], rn[u]);
+  PT_SIDE(7);
+  PtF2 xo_[CNT], xn_[CNT];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) {
+    const int j = 2 * (p0 + (BEGIN + u) * L);
+    float oa, ob, na, nb;
+    pt_f2_split(ro[u], oa, ob);
+    pt_f2_split(rn[u], na, nb);
+    const bool sa = j == m, sb = j + 1 == m;
+    oa = sa ? lj.rc2 : fminf(oa, lj.rc2); na = sa ? lj.rc2 : fminf(na, lj.rc2);
+    ob = sb ? lj.rc2 : fminf(ob, lj.rc2); nb = sb ? lj.rc2 : fminf(nb, lj.rc2);
+#if PT_F32_ONE_RCP
+    // one reciprocal for the old and the new distance of a partner: 1/r_o^2 = r_n^2 / (r_o^2 r_n^2)
+    const PtF2 co = pt_f2(oa, ob), cn = pt_f2(na, nb);
+    float pa, pb;
+    pt_f2_split(pt_mul2(co, cn), pa, pb);
+    const PtF2 ip = pt_f2(PtNum<float>::rcp(pa), PtNum<float>::rcp(pb));
+    xo_[u] = pt_mul2(ip, cn);
+    xn_[u] = pt_mul2(ip, co);
+#else
+    xo_[u] = pt_f2(PtNum<float>::rcp(oa), PtNum<float>::rcp(ob));
+    xn_[u] = pt_f2(PtNum<float>::rcp(na), PtNum<float>::rcp(nb));
+#endif
+  }
+  PT_SIDE(8);
+  PT_SIDE(9);
+  PT_SIDE(10);
+  PtF2 eo[CNT], en[CNT];
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) { eo[u] = pt_mul2(xo_[u], xo_[u]); en[u] = pt_mul2(xn_[u], xn_[u]); }
+  PT_SIDE(11);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) { xo_[u] = pt_fma2(eo[u], xo_[u], mhc2); xn_[u] = pt_fma2(en[u], xn_[u], mhc2); }   // v = 1/r^6 - c/2
+  PT_SIDE(12);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) { eo[u] = pt_sub2(xn_[u], xo_[u]); en[u] = pt_add2(xn_[u], xo_[u]); }
+  PT_SIDE(13);
+#pragma unroll
+  for (int u = 0; u < CNT; ++u) acc[(BEGIN + u) & 1] = pt_fma2(eo[u], en[u], acc[(BEGIN + u) & 1]);
+#undef PT_SIDE
+}
+
+// NI2 iterations of two partners each (2 L NI2 table slots); returns this lane's share of Delta E_LJ
+template <int L, int NI2, int LEVG>
+__device__ __forceinline__ float pair_groups_f2(const PtLJ<float>& lj, const PtCoords<float>& X, int lig, int m, float xo,
+                                                float yo, float zo, float tdx, float tdy, float tdz, float dd,
+                                                BondChain<float>& side)
+{
+  constexpr int P = kGroupPoints;
+  constexpr int NG = n_groups(NI2);
+  static_assert(NG >= 1 && NG <= 4, "add a group");
+  PtF2 acc[2] = {pt_f2(0.0f, 0.0f), pt_f2(0.0f, 0.0f)};
+  const PtF2 xo2 = pt_f2(xo, xo), yo2 = pt_f2(yo, yo), zo2 = pt_f2(zo, zo), tdx2 = pt_f2(tdx, tdx), tdy2 = pt_f2(tdy, tdy),
+             tdz2 = pt_f2(tdz, tdz), dd2 = pt_f2(dd, dd), mhc2 = pt_f2(lj.mhc, lj.mhc);
+#define PT_PG(g)                                                                                              \
+  if (NG > g)                                                                                                 \
+    pair_group_f2<L, group_begin(NI2, g < NG ? g : 0), group_size(NI2, g < NG ? g : 0), g * P, NG * P, LEVG>(   \
+        lj, X, lig, m, xo2, yo2, zo2, tdx2, tdy2, tdz2, dd2, mhc2, acc, side)
+  PT_PG(0);
+  PT_PG(1);
+  PT_PG(2);
+  PT_PG(3);
+#undef PT_PG
+  float a0, a1, b0, b1;
+  pt_f2_split(acc[0], a0, a1);
+  pt_f2_split(acc[1], b0, b1);
+  return lj.A * ((a0 + a1) + (b0 + b1));
+}
+
 // ------------------------------------------------------------------------------------------
 // Warp-group kernel: L lanes per chain, 32/L chains per warp (L >= 8: roles 0..4 need 5 lanes).
 // ------------------------------------------------------------------------------------------
@@ -310,14 +422,18 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
 // `smem0` (stride `sstride` Reals between chains, Ns slots per coordinate array).  `delay`: cycles to
 // wait before the first step (phase stagger).
 template <typename Real, int L, int NI, bool TRACE>
-__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns, int chain0, int chain_end,
-                                           int delay, const uint32_t t0, const int n_sweeps)
+__device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstride, int Ns_runtime, int chain0,
+                                           int chain_end, int delay, const uint32_t t0, const int n_sweeps)
 {
   static_assert(L >= 8 && L <= 32, "lanes per chain");
   constexpr int G = 32 / L;
   // Short partner loops have fewer stage points than the bond stream has levels: one level per point,
   // the rest of the stream runs behind the reduction of the pair sums (latency-bound shapes).
-  constexpr int NPTS = n_groups(NI) * kGroupPoints;
+  constexpr bool F2 = sizeof(Real) == 4 && NI > 0;      // fp32: two partners per lane and iteration (pair_group_f2)
+  constexpr int NI2 = (NI + 1) / 2;
+  constexpr int NPTS = n_groups(F2 ? NI2 : NI) * kGroupPoints;
+  // table slots per coordinate array: unrolled kernels know them at compile time (fp32: an even number of iterations)
+  const int Ns = NI > 0 ? (F2 ? 2 * L * NI2 : L * NI) : Ns_runtime;
   constexpr bool TAIL = NI > 0 && (L & (L - 1)) == 0 && NPTS < BondChain<Real>::NLEV;
   constexpr int LEVG = TAIL ? NPTS : BondChain<Real>::NLEV;
   // lanes beyond G L (L = 10: lanes 30, 31) are ghosts: they repeat the last real lane and nobody reads them
@@ -380,7 +496,8 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
       bc.xo = xo; bc.yo = yo; bc.zo = zo; bc.xn = xn; bc.yn = yn; bc.zn = zn; bc.u = p.u;
       Real part;
       if (NI > 0) {
-        part = pair_groups<Real, L, (NI > 0 ? NI : 1), LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
+        if constexpr (F2) part = pair_groups_f2<L, NI2, LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
+        else part = pair_groups<Real, L, (NI > 0 ? NI : 1), LEVG>(lj, X, lig, m, xo, yo, zo, tdx, tdy, tdz, dd, bc);
       } else {
         bc.run_all();
         Real en = (Real)0, eo = (Real)0;
