@@ -271,10 +271,20 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
 #define PT_MAXGROUP 5
 #endif
 constexpr int kMaxGroup = PT_MAXGROUP;
-__host__ __device__ constexpr int n_groups(int NI) { return NI <= 0 ? 0 : (NI + kMaxGroup - 1) / kMaxGroup; }
+#ifndef PT_MAXGROUP_F2
+#define PT_MAXGROUP_F2 5
+#endif
+constexpr int kMaxGroupF2 = PT_MAXGROUP_F2;   // fp32: pairs of partners per group
+__host__ __device__ constexpr int n_groups(int NI, int mg = kMaxGroup) { return NI <= 0 ? 0 : (NI + mg - 1) / mg; }
 // size and first iteration of group g: the first (NI mod n) groups get one more
-__host__ __device__ constexpr int group_size(int NI, int g) { return NI / n_groups(NI) + (g < NI % n_groups(NI) ? 1 : 0); }
-__host__ __device__ constexpr int group_begin(int NI, int g) { return g == 0 ? 0 : group_begin(NI, g - 1) + group_size(NI, g - 1); }
+__host__ __device__ constexpr int group_size(int NI, int g, int mg = kMaxGroup)
+{
+  return NI / n_groups(NI, mg) + (g < NI % n_groups(NI, mg) ? 1 : 0);
+}
+__host__ __device__ constexpr int group_begin(int NI, int g, int mg = kMaxGroup)
+{
+  return g == 0 ? 0 : group_begin(NI, g - 1, mg) + group_size(NI, g - 1, mg);
+}
 
 // The whole partner loop of NI > 0 iterations: returns this lane's share of Delta E_LJ.
 // s0 = this lane's first partner, sm = the moved monomer (its own slot is masked out).
@@ -392,14 +402,14 @@ __device__ __forceinline__ float pair_groups_f2(const PtLJ<float>& lj, const PtC
                                                 BondChain<float>& side)
 {
   constexpr int P = kGroupPoints;
-  constexpr int NG = n_groups(NI2);
+  constexpr int NG = n_groups(NI2, kMaxGroupF2);
   static_assert(NG >= 1 && NG <= 4, "add a group");
   PtF2 acc[2] = {pt_f2(0.0f, 0.0f), pt_f2(0.0f, 0.0f)};
   const PtF2 xo2 = pt_f2(xo, xo), yo2 = pt_f2(yo, yo), zo2 = pt_f2(zo, zo), tdx2 = pt_f2(tdx, tdx), tdy2 = pt_f2(tdy, tdy),
              tdz2 = pt_f2(tdz, tdz), dd2 = pt_f2(dd, dd), mhc2 = pt_f2(lj.mhc, lj.mhc);
 #define PT_PG(g)                                                                                              \
   if (NG > g)                                                                                                 \
-    pair_group_f2<L, group_begin(NI2, g < NG ? g : 0), group_size(NI2, g < NG ? g : 0), g * P, NG * P, LEVG>(   \
+    pair_group_f2<L, group_begin(NI2, g < NG ? g : 0, kMaxGroupF2), group_size(NI2, g < NG ? g : 0, kMaxGroupF2), g * P, NG * P, LEVG>(   \
         lj, X, lig, m, xo2, yo2, zo2, tdx2, tdy2, tdz2, dd2, mhc2, acc, side)
   PT_PG(0);
   PT_PG(1);
@@ -431,7 +441,7 @@ __device__ __forceinline__ void sweep_warp(const PtDev& d, Real* smem0, int sstr
   // the rest of the stream runs behind the reduction of the pair sums (latency-bound shapes).
   constexpr bool F2 = sizeof(Real) == 4 && NI > 0;      // fp32: two partners per lane and iteration (pair_group_f2)
   constexpr int NI2 = (NI + 1) / 2;
-  constexpr int NPTS = n_groups(F2 ? NI2 : NI) * kGroupPoints;
+  constexpr int NPTS = (F2 ? n_groups(NI2, kMaxGroupF2) : n_groups(NI)) * kGroupPoints;
   // table slots per coordinate array: unrolled kernels know them at compile time (fp32: an even number of iterations)
   const int Ns = NI > 0 ? (F2 ? 2 * L * NI2 : L * NI) : Ns_runtime;
   constexpr bool TAIL = NI > 0 && (L & (L - 1)) == 0 && NPTS < BondChain<Real>::NLEV;
