@@ -61,7 +61,7 @@ struct PtLaunch {
   int sstride;         // shared-memory stride between chains, in Reals
   int Ns;              // padded monomers per coordinate array in shared memory
   int ni;              // unrolled partner-loop iterations of the chosen kernel (0 = run-time loop)
-  int kind;            // PT_K_GROUP, PT_K_COMP or PT_K_CTA
+  int kind;            // PT_K_GROUP, PT_K_COMP, PT_K_CTA, PT_K_SEVEN(_FULL) or PT_K_WS (then lanes = 32 x pair warps)
   int stagger;         // PT_K_GROUP: start delay in cycles per rank of a warp on its sub-partition (0 = none)
   // PT_K_COMP / PT_K_SEVEN: warps of different kinds in one CTA; kind 0, 1, 2, 3 = 8, 16, 32, 10 lanes per chain
   // (k_sweep_comp uses 0..2; k_sweep_seven 0 for warps 0..3 and 3 for warps 4..7)
@@ -74,10 +74,12 @@ struct PtLaunch {
   int wdelay[8];       // start delay of warp w in cycles
 };
 
-enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4 };
+enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4, PT_K_WS = 5 };
 
 // Kernel tables, one per translation unit that instantiates sweep kernels (nullptr = not in this unit).
 PtSweepFn pt_lookup_group(int lanes, int ni, int precision, bool trace);   // pt_sweep_group.cu
+PtSweepFn pt_lookup_ws(int pair_warps, int ni, int precision, bool trace);   // pt_sweep_ws.cu
+int pt_ws_variant(int pair_warps, int ni_needed);                          // smallest instantiated NI >= ni_needed, or -1
 PtSweepFn pt_lookup_cta(int precision, bool trace);                        // pt_sweep_group.cu
 PtSweepFn pt_lookup_comp(int kind, const int nik[4], int precision, bool trace);   // pt_sweep_comp*.cu
 // the unrolled variants of k_sweep_group: smallest NI >= ni_needed for this lane count, 0 = run-time loop

@@ -56,6 +56,7 @@ int stagger_cycles(int ni) { return (int)(2.1 * (26.0 * ni + 70.0)); }
 PtSweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return pt_lookup_cta(precision, trace);
+  if (pl.kind == PT_K_WS) return pt_lookup_ws(pl.lanes / 32, pl.ni, precision, trace);
   if (pl.kind == PT_K_COMP || pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
     return pt_lookup_comp(pl.kind, pl.nik, precision, trace);
   return pt_lookup_group(pl.lanes, pl.ni, precision, trace);
@@ -148,6 +149,35 @@ bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch*
   return true;
 }
 
+// Warp-specialised CTA per chain (k_sweep_ws): P pair warps + one stream warp, every warp alone on its SM
+// sub-partition.  Sequential order only, N >= 4.  P grows with the chain length (the pair warps' share of a step is
+// about 60 cycles per partner iteration beside ~300 for load, reduce, decide; the stream warp needs ~420), as far as
+// the sub-partitions last.
+bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLaunch* out)
+{
+  if (d.select_mode != PT_SEQUENTIAL || d.N < 5) return false;
+  for (int P = d.N > 192 ? 3 : (d.N > 64 ? 2 : 1); P >= 1; --P) {
+    if ((long long)d.C * (P + 1) > smsp) continue;
+    const int T = 32 * P;
+    const int ni = pt_ws_variant(P, (d.N + T - 1) / T);
+    if (ni < 0) continue;
+    PtLaunch pl{};
+    pl.kind = PT_K_WS;
+    pl.lanes = T;
+    pl.ni = ni;
+    pl.Ns = table_slots(T, ni, real_bytes);
+    pl.sstride = 3 * pl.Ns;
+    pl.threads = 32 * (P + 2);
+    pl.chains_per_cta = 1;
+    pl.grid = d.C;
+    pl.smem_bytes = pl.sstride * real_bytes;
+    if (!kernel_of(pl, precision, false)) continue;
+    *out = pl;
+    return true;
+  }
+  return false;
+}
+
 }  // namespace
 
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan)
@@ -170,6 +200,8 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     // More chains than SM sub-partitions: composed CTAs, chains spread evenly over the SMs (no staircase in
     // the number of replicas beyond the one of the most loaded sub-partition).
     if ((long long)d.C > smsp) done = plan_comp(d, precision, real_bytes, sms, &pl);
+    // Few chains: a step is as long as its dependence chain; a second warp takes the bond stream off it.
+    if (!done) done = plan_ws(d, precision, real_bytes, smsp, &pl);
     if (!done) {
       // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
       // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
@@ -237,6 +269,7 @@ void pt_sweep_kernel_desc(const PtLaunch& pl, int precision, bool trace, char* b
 {
   const char* real = precision == PT_F32 ? "float" : "double";
   if (pl.kind == PT_K_CTA) snprintf(buf, n, "k_sweep_cta<%s,threads=%d,trace=%d>", real, pl.threads, trace ? 1 : 0);
+  else if (pl.kind == PT_K_WS) snprintf(buf, n, "k_sweep_ws<%s,%d,%d,trace=%d>", real, pl.lanes / 32, pl.ni, trace ? 1 : 0);
   else if (pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
     snprintf(buf, n, "k_sweep_seven<%s,%d,%d,%s,trace=%d>", real, pl.nik[0], pl.nik[3],
              pl.kind == PT_K_SEVEN_FULL ? "full" : "partial", trace ? 1 : 0);
@@ -250,6 +283,7 @@ cudaError_t pt_launch_sweep(const PtDev& d, int precision, const PtLaunch& pl, u
 {
   PtSweepFn fn = kernel_of(pl, precision, d.tr_move != nullptr);
   if (!fn) return cudaErrorInvalidValue;
+  if (n_sweeps <= 0) return cudaSuccess;
   fn<<<dim3(pl.grid), dim3(pl.threads), pl.smem_bytes, stream>>>(d, pl, t0, n_sweeps);
   return cudaGetLastError();
 }

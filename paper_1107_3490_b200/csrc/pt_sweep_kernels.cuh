@@ -191,10 +191,10 @@ constexpr int kGroupPoints = 14;   // stage points per pair group
 // shift C needs the count of inside pairs (one predicated add); A and C are applied once per step by the
 // caller.  The new squared distance follows from the old one:
 // |b + delta|^2 = |b|^2 + 2 delta.b + |delta|^2, b = x_m - x_j.
-template <typename Real, int L, int NI, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
+template <typename Real, int L, int NI, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG, class Side>
 __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
                                            Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
-                                           Real (&acc)[4], int& cnt, BondChain<Real>& side)
+                                           Real (&acc)[4], int& cnt, Side& side)
 {
 #define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
   Real bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
@@ -288,10 +288,10 @@ __host__ __device__ constexpr int group_begin(int NI, int g, int mg = kMaxGroup)
 
 // The whole partner loop of NI > 0 iterations: returns this lane's share of Delta E_LJ.
 // s0 = this lane's first partner, sm = the moved monomer (its own slot is masked out).
-template <typename Real, int L, int NI, int LEVG>
+template <typename Real, int L, int NI, int LEVG, class Side>
 __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords<Real>& X, int s0, int sm,
                                             Real xo, Real yo, Real zo, Real tdx, Real tdy, Real tdz, Real dd,
-                                            BondChain<Real>& side)
+                                            Side& side)
 {
   constexpr int P = kGroupPoints;
   constexpr int NG = n_groups(NI);
@@ -321,10 +321,10 @@ __device__ __forceinline__ Real pair_groups(const PtLJ<Real>& lj, const PtCoords
 // u = u_c in the old and in the new position and (v_n - v_o)(v_n + v_o) is exactly 0 -- no mask, no count of inside
 // pairs, and C drops out.  The moved monomer itself gets r^2 = r_c^2 in both positions.  (The fp64 path cannot clamp:
 // it has no single-instruction 64-bit minimum.)  The fp32 path is checked statistically (tests/test_gpu_fp32_stat.py).
-template <int L, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG>
+template <int L, int BEGIN, int CNT, int PBASE, int NPTS, int LEVG, class Side>
 __device__ __forceinline__ void pair_group_f2(const PtLJ<float>& lj, const PtCoords<float>& X, int p0, int m, PtF2 xo2,
                                               PtF2 yo2, PtF2 zo2, PtF2 tdx2, PtF2 tdy2, PtF2 tdz2, PtF2 dd2, PtF2 mhc2,
-                                              PtF2 (&acc)[2], BondChain<float>& side)
+                                              PtF2 (&acc)[2], Side& side)
 {
 #define PT_SIDE(n) side.template run<PBASE + (n), NPTS, LEVG>()
   PtF2 bx[CNT], by[CNT], bz[CNT], ro[CNT], rn[CNT];
@@ -396,10 +396,10 @@ __device__ __forceinline__ void pair_group_f2(const PtLJ<float>& lj, const PtCoo
 }
 
 // NI2 iterations of two partners each (2 L NI2 table slots); returns this lane's share of Delta E_LJ
-template <int L, int NI2, int LEVG>
+template <int L, int NI2, int LEVG, class Side>
 __device__ __forceinline__ float pair_groups_f2(const PtLJ<float>& lj, const PtCoords<float>& X, int lig, int m, float xo,
                                                 float yo, float zo, float tdx, float tdy, float tdz, float dd,
-                                                BondChain<float>& side)
+                                                Side& side)
 {
   constexpr int P = kGroupPoints;
   constexpr int NG = n_groups(NI2, kMaxGroupF2);

@@ -1,0 +1,33 @@
+// k_sweep_ws instantiations: the warp-specialised kernel of the latency-bound shapes (pt_sweep_ws.cuh).
+#include "pt_sweep_ws.cuh"
+
+namespace {
+
+struct WsVariant {
+  int P, NI;                  // pair warps, partner iterations per pair thread (32 P NI table slots)
+  PtSweepFn f64[2], f32[2];   // [0] timed, [1] with the decision trace
+};
+
+#define PT_WS(P, NI)                                                            \
+  { P, NI, { k_sweep_ws<double, P, NI, false>, k_sweep_ws<double, P, NI, true> }, \
+    { k_sweep_ws<float, P, NI, false>, k_sweep_ws<float, P, NI, true> } }
+const WsVariant kWs[] = {
+    PT_WS(1, 1), PT_WS(1, 2), PT_WS(1, 3), PT_WS(1, 4), PT_WS(2, 2), PT_WS(2, 3), PT_WS(3, 3), PT_WS(3, 4), PT_WS(3, 5),
+};
+
+}  // namespace
+
+// smallest instantiated NI >= ni_needed for P pair warps, or -1
+int pt_ws_variant(int pair_warps, int ni_needed)
+{
+  for (const WsVariant& v : kWs)
+    if (v.P == pair_warps && v.NI >= ni_needed) return v.NI;
+  return -1;
+}
+
+PtSweepFn pt_lookup_ws(int pair_warps, int ni, int precision, bool trace)
+{
+  for (const WsVariant& v : kWs)
+    if (v.P == pair_warps && v.NI == ni) return precision == PT_F32 ? v.f32[trace ? 1 : 0] : v.f64[trace ? 1 : 0];
+  return nullptr;
+}

@@ -1,0 +1,287 @@
+// Warp-specialised sweep kernel for the latency-bound shapes: few chains (at most one warp per SM sub-partition
+// even with P + 1 warps per chain), sequential monomer order.  One CTA per chain:
+//
+//   warps 0 .. P-1  "pair warps"   A3 for their share of the partners (32 P threads stride over the table, the
+//                                  unrolled stage-major groups of pt_sweep_kernels.cuh), warp-reduce, one partial
+//                                  sum per warp into shared memory; after the step's barrier EVERY pair thread
+//                                  adds the partials and the bond terms, decides (A6) and keeps the books; the
+//                                  thread that owns the moved monomer's table slot commits (A7);
+//   warp P          "stream warp"  A5 (Eq. 3: sqrt and log of up to four bonds) and log u, as plain serial code,
+//                                  ONE STEP AHEAD and for both outcomes of the step in flight.
+//
+// Why.  With one warp per chain (k_sweep_group) a step is as long as its dependence chain
+//   commit -> load -> [pair stages | sqrt, log: ~30 dependent fp64 levels] -> reduce -> decide -> commit
+// and the serial stream is the longest part of it (720-1270 cycles per step on BASELINE configs 1-4, of which the
+// pair arithmetic needs 100-600).  A second warp can take the stream off that chain only if it does not wait for
+// the decision.  In the sequential order it need not: the stream of step g + 1 (monomer m' = m + 1) depends on
+// step g only through the position of m, the left bond neighbour of m', and that position is one of two known
+// candidates.  Roles of the stream warp's lanes (bit 0: right neighbour, bit 1: old position of m', bit 2: step g
+// rejected):
+//   0  new bond (m', m'-1), step g accepted      4  the same, rejected
+//   2  old bond (m', m'-1), accepted             6  the same, rejected
+//   1  new bond (m', m'+1)     3  old bond (m', m'+1)     5  log u
+// "accepted" takes x_m' = x_m + delta from registers, "rejected" reads the table, which holds the old position of m
+// until the step's barrier.  One shuffle level leaves b0 + b2, b1 + b3 and b4 + b6 in lanes 0, 1, 4; they go to a
+// four-deep ring in shared memory together with log u and the ballot of the broken new bonds, and the deciders of
+// step g + 1 pick the sums that belong to the outcome of step g.
+//
+// One named barrier per step (all P + 1 warps): partial sums and the stream record of the step are complete.
+// No barrier is needed after the commit: a table slot is read in the pair loop by one thread only, its owner, and
+// the owner is the thread that commits; the stream warp reads slots m', m' +- 1 while slot m - 1 may be committed
+// (distinct for N >= 4); the moved monomer itself is read again N steps later.
+// The paper's own mapping is one block per replica; this is that mapping with the block's warps
+// given different work.  Random-pick mode, N < 4 and larger batches keep the other kernels (pt_plan_sweep).
+#pragma once
+#include "pt_sweep_kernels.cuh"
+
+namespace {
+
+// the pair groups' side stream is empty here
+struct PtNoSide {
+  template <int P, int NPTS, int LEVG> __device__ __forceinline__ void run() {}
+};
+
+__device__ __forceinline__ void pt_bar_sync(int id, int nthreads)
+{
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void pt_bar_arrive(int id, int nthreads)
+{
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// ring of stream records: [slot][0..3] = b0 + b2 ("accepted" left bond terms), b1 + b3 (right bond terms),
+// b4 + b6 ("rejected" left bond terms), log u;  mask = ballot of broken NEW bonds (bits 0, 1, 4)
+struct PtWsShared {
+  double rec[4][4];
+  unsigned mask[4];
+  double red[2][4];   // partial pair sums of the pair warps, double-buffered by step parity
+};
+
+// log(v), v normal and > 0: PtNum<double>::log_ with the series by Estrin's scheme (depth 4 instead of 10), the
+// arithmetic of BondChain's levels 15..29
+template <typename Real> __device__ __forceinline__ Real ws_log(Real v)
+{
+  if constexpr (sizeof(Real) == 8) {
+    const int hi = __double2hiint(v);
+    const int ex = (hi - 0x3fe6a09e) >> 20;
+    const double mm = __hiloint2double(hi - (ex << 20), __double2loint(v));
+    const double de = (double)ex;
+    const double f = mm - 1.0, mp = mm + 1.0;
+    double x = PtNum<double>::rcp_seed(mp);
+    double e = fma(-mp, x, 1.0);
+    e = fma(e, e, e);
+    x = fma(x, e, x);
+    const double sv = f * x;
+    const double z = sv * sv, s2 = sv + sv;
+    const double p01 = fma(kPtLogC[1], z, kPtLogC[0]), p23 = fma(kPtLogC[3], z, kPtLogC[2]);
+    const double p45 = fma(kPtLogC[5], z, kPtLogC[4]), p67 = fma(kPtLogC[7], z, kPtLogC[6]);
+    const double p89 = fma(kPtLogC[9], z, kPtLogC[8]), z2 = z * z;
+    double q0 = fma(p23, z2, p01);
+    const double q1 = fma(p67, z2, p45), z4 = z2 * z2;
+    q0 = fma(q1, z4, q0);
+    q0 = fma(p89, z4 * z4, q0);
+    double lg = fma(sv, q0 * z, s2);
+    lg = fma(de, 0x1.abc9e3b39803fp-56, lg);
+    return fma(de, 0x1.62e42fefa39efp-1, lg);
+  } else {
+    return PtNum<float>::log_(v);
+  }
+}
+
+// One pass of the stream for monomer m (old position xo.., proposed xn.., uniform u).  `ahead`: lanes 0 and 2
+// take the left neighbour at its proposed position, table entry + (ex, ey, ez), instead of the table entry
+// (the same separately rounded addition as the proposal itself, R7).
+template <typename Real>
+__device__ __forceinline__ void ws_stream(const PtDev& d, const PtCoords<Real>& X, int lane, int m, int N, Real xo, Real yo,
+                                          Real zo, Real xn, Real yn, Real zn, Real u, bool ahead, Real ex, Real ey,
+                                          Real ez, PtWsShared& sh, int slot)
+{
+  const int role = lane;
+  const int nb = (role & 1) ? m + 1 : m - 1;
+  const bool isbond = role < 7 && role != 5 && nb >= 0 && nb < N;
+  const bool isnew = (role & 2) == 0;
+  const bool moved = ahead && (role == 0 || role == 2);
+  Real xb, yb, zb;
+  X.get(isbond ? nb : m, xb, yb, zb);
+  xb = PtNum<Real>::shift(xb, moved ? ex : (Real)0);
+  yb = PtNum<Real>::shift(yb, moved ? ey : (Real)0);
+  zb = PtNum<Real>::shift(zb, moved ? ez : (Real)0);
+  const Real dx = (isnew ? xn : xo) - xb;
+  const Real dy = (isnew ? yn : yo) - yb;
+  const Real dz = (isnew ? zn : zo) - zb;
+  const Real r2 = isbond ? fma(dz, dz, fma(dy, dy, dx * dx)) : (Real)(d.r0 * d.r0);
+  const Real r = PtNum<Real>::sqrt_(r2);
+  const Real q = (r - (Real)d.r0) * (Real)d.invR;
+  const Real gq = fma(-q, q, (Real)1);              // 1 - ((r - r0)/R)^2, Eq. (3)
+  const bool in_range = gq > (Real)0;               // false for NaN as well
+  const bool broke = isbond && isnew && !in_range;
+  const Real arg = role == 5 ? u : ((isbond && in_range) ? gq : (Real)1);
+  const Real lg = ws_log<Real>(arg);
+  const Real fc = isnew ? (Real)d.feneC : (Real)-d.feneC;   // -(K/2) R^2
+  const Real bond = role != 5 ? fc * lg : (Real)0;
+  const Real pairsum = bond + __shfl_xor_sync(0xffffffffu, bond, 2);
+  const unsigned mask = __ballot_sync(0xffffffffu, broke);
+  // lanes 0, 1, 4, 5 -> rec[slot][0, 1, 2, 3]; one predicated store each (a chain of ifs becomes a jump table)
+  const int idx = lane == 0 ? 0 : (lane == 1 ? 1 : (lane == 4 ? 2 : 3));
+  const bool writes = ((0x33u >> lane) & 1u) != 0u && lane < 8;
+  const double val = lane == 5 ? (double)lg : (double)pairsum;
+  if (writes) sh.rec[slot][idx] = val;
+  if (lane == 2) sh.mask[slot] = mask;
+}
+
+template <typename Real, int P, int NI, bool TRACE>
+__global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, const PtLaunch pl, const uint32_t t0,
+                                                           const int n_sweeps)
+{
+  static_assert(P >= 1 && P <= 3 && NI >= 1, "pair warps and partner iterations");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ PtWsShared sh;
+  constexpr int T = 32 * P;                               // pair threads
+  constexpr int NT = 32 * (P + 2);                        // + two stream warps
+  constexpr bool F2 = sizeof(Real) == 4;                  // fp32: two partners per thread and iteration
+  constexpr int NI2 = (NI + 1) / 2;
+  constexpr int Ns = F2 ? 2 * T * NI2 : T * NI;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int N = d.N;
+  const int total = n_sweeps * N;
+
+  ChainCtx c;
+  ctx_load(d, blockIdx.x, d.C, c);
+  const Real width = (Real)d.width[c.i];
+  const PtCoords<Real> X(reinterpret_cast<Real*>(smem_raw), Ns);
+
+  // A1: HBM -> shared memory; padding entries lie far outside every cutoff
+  Real* gx = reinterpret_cast<Real*>(d.coords) + (size_t)c.s * 3 * d.Ng;
+  for (int j = tid; j < Ns; j += NT) {
+    const bool in = j < N;
+    X.set(j, in ? gx[j] : (Real)PT_FAR, in ? gx[d.Ng + j] : (Real)PT_FAR, in ? gx[2 * d.Ng + j] : (Real)PT_FAR);
+  }
+  __syncthreads();
+
+  if (warp >= P) {
+    // ---- stream warps: warp P takes the even steps, warp P + 1 the odd ones ----
+    // The stream of step g needs nothing that steps g - 2 and g - 1 decide (only the two candidates for the left
+    // neighbour, the monomer of step g - 1), so it has two steps' time: the warp arrives at the barrier of step
+    // g - 2 without waiting and waits at the barrier of step g - 1, after which its record is complete.  Two
+    // barrier ids alternate with the step parity, so an arrival can never be counted for the wrong step.
+    const int s = warp - P;
+    int blk_no = -1;
+    DrawBlock<Real> blk;
+    auto numbers = [&](int g) {   // the draw of step g (steps are asked for in increasing order)
+      if ((g >> 3) != blk_no) {
+        blk_no = g >> 3;
+        blk = draw_block<Real>(c, false, N, width, t0, g & ~7, lane);
+      }
+      return draw_fetch<Real>(blk, g, 0u);
+    };
+    for (int g = s; g <= total; g += 2) {
+#ifdef PT_WS_DEBUG
+      if (blockIdx.x == 0 && lane == 0 && g < 8) printf("stream warp %d iteration %d\n", s, g);
+#endif
+      if (g >= 2) pt_bar_arrive(1 + (g & 1), NT);                    // barrier of step g - 2
+      Real ex = (Real)0, ey = (Real)0, ez = (Real)0;
+      if (g >= 1) { const DrawBlock<Real> pv = numbers(g - 1); ex = pv.dx; ey = pv.dy; ez = pv.dz; }
+      const DrawBlock<Real> nx = numbers(g);
+      Real xa, ya, za;
+      X.get(nx.m, xa, ya, za);
+      const Real xp = PtNum<Real>::shift(xa, nx.dx), yp = PtNum<Real>::shift(ya, nx.dy), zp = PtNum<Real>::shift(za, nx.dz);
+      ws_stream<Real>(d, X, lane, nx.m, N, xa, ya, za, xp, yp, zp, nx.u, g >= 1, ex, ey, ez, sh, g & 3);
+      if (g < 2) {
+        __syncthreads();                                            // the records of steps 0 and 1 precede the loop
+        // barrier of step 0: waited for, not just arrived at -- this warp's next operation on the same id is the
+        // wait of step 2, and an arrival must never be counted for an earlier step than it is meant for
+        if (g == 1) pt_bar_sync(1, NT);
+      } else {
+        pt_bar_sync(1 + ((g - 1) & 1), NT);                         // barrier of step g - 1
+      }
+    }
+    // the loop ends with g = total or total - 1; in the second case the barrier of the last step is still owed
+    if ((((total - s) & ~1) + s) == total - 1) pt_bar_arrive(1 + ((total - 1) & 1), NT);
+    return;
+  }
+
+  // ---- pair warps ----
+  __syncthreads();
+  DrawBlock<Real> blk = draw_block<Real>(c, false, N, width, t0, 0, lane);
+  DrawBlock<Real> nx = draw_fetch<Real>(blk, 0, 0u);
+  const PtLJ<Real> lj(d);
+  const double nbeta = -c.beta;
+  PtNoSide noside;
+  bool acc_prev = true;
+  int gstep = 0;
+  for (int sw = 0; sw < n_sweeps; ++sw) {
+    const uint32_t t = t0 + (uint32_t)sw;
+    for (int k = 0; k < N; ++k) {
+      // A2: this step's numbers were fetched one step ahead
+      const DrawBlock<Real> p = nx;
+      const int g = gstep;
+      ++gstep;
+      if ((gstep & 7) == 0) blk = draw_block<Real>(c, false, N, width, t0, gstep, lane);
+      nx = draw_fetch<Real>(blk, gstep, 0u);
+      const int m = p.m;
+      Real xo, yo, zo;
+      X.get(m, xo, yo, zo);
+      const Real xn = PtNum<Real>::shift(xo, p.dx);
+      const Real yn = PtNum<Real>::shift(yo, p.dy);
+      const Real zn = PtNum<Real>::shift(zo, p.dz);
+      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
+      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
+      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
+
+      // A3: this thread's partners
+      Real part;
+      if constexpr (F2) part = pair_groups_f2<T, NI2, 1>(lj, X, tid, m, xo, yo, zo, tdx, tdy, tdz, dd, noside);
+      else part = pair_groups<Real, T, NI, 1>(lj, X, tid, m, xo, yo, zo, tdx, tdy, tdz, dd, noside);
+      // A4: warp sum, one partial per warp
+      part = group_sum<Real, 32>(part, lane, 0);
+      if (lane == 0) sh.red[g & 1][warp] = (double)part;
+#ifdef PT_WS_DEBUG
+      if (blockIdx.x == 0 && lane == 0 && g < 6) printf("pair warp %d before barrier %d\n", warp, g);
+#endif
+      pt_bar_sync(1 + (g & 1), NT);   // partial sums and the stream record of this step are complete
+#ifdef PT_WS_DEBUG
+      if (blockIdx.x == 0 && lane == 0 && g < 6) printf("pair warp %d after barrier %d\n", warp, g);
+#endif
+
+      double dEd = sh.red[g & 1][0];
+      if (P > 1) dEd += sh.red[g & 1][1];
+      if (P > 2) dEd += sh.red[g & 1][2];
+      const int slot = g & 3;
+      dEd += sh.rec[slot][1];
+      dEd += acc_prev ? sh.rec[slot][0] : sh.rec[slot][2];
+      const double logu = sh.rec[slot][3];
+      const bool bond_broken = (sh.mask[slot] & (acc_prev ? 0x03u : 0x12u)) != 0u;
+      const Real dE = (Real)dEd;
+
+      // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
+      const bool accept = !bond_broken && (dE <= (Real)0 || logu < nbeta * (double)dE);
+
+      // A7: commit by the owner of the table slot (the only thread whose pair loop reads it)
+      const int owner = F2 ? (m >> 1) % T : m % T;
+      if (accept && tid == owner) X.set(m, xn, yn, zn);
+      if (TRACE) {   // test support (pt_set_trace): a separate instantiation
+        if (tid == 0 && d.tr_move && (long long)t < d.cap_sweeps)
+          d.tr_move[((size_t)c.ti * d.cap_sweeps + t) * (size_t)N + k] = accept ? 1 : 0;
+      }
+      c.erun += accept ? (double)dE : 0.0;
+      c.acc += accept ? 1u : 0u;
+      c.brej += bond_broken ? 1u : 0u;
+      acc_prev = accept;
+    }
+
+    // A8: measurement once per sweep; the last commit may have come from another pair warp
+    if (P > 1) pt_bar_sync(3, T);
+    else __syncwarp();
+    if (d.observables && warp == 0) measure_shape<Real, 32>(d, c, N, lane, 0, X);
+    if (tid == 0) measure_energy(d, c, t);
+  }
+
+  // A9: shared memory -> HBM
+  if (P > 1) pt_bar_sync(3, T);
+  else __syncwarp();
+  for (int j = tid; j < N; j += T) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
+  if (tid == 0) ctx_store(d, c, n_sweeps);
+}
+
+}  // namespace

@@ -66,9 +66,24 @@ def test_config3_full_run():
 
 
 def test_config4_full_run():
-    """N=309, M=128, all 2000 sweeps, default mapping: one warp per replica (10 unrolled partner iterations)."""
-    rep, g, _ = _both(synth.make_inputs(4), 2000, nbins=4096, expect_kernel="k_sweep_group<double,32,10,")
-    assert g[0]["launch_info"]["lanes"] == 32 and g[0]["counters"] == (2000, 100)
+    """N=309, M=128, all 2000 sweeps, default mapping: one CTA per replica, three pair warps (4 partner iterations
+    each) and two stream warps (k_sweep_ws)."""
+    rep, g, _ = _both(synth.make_inputs(4), 2000, nbins=4096, expect_kernel="k_sweep_ws<double,3,4,")
+    assert g[0]["launch_info"]["lanes"] == 96 and g[0]["counters"] == (2000, 100)
+
+
+def test_config4_one_warp_per_replica():
+    """Config 4 on the mapping that was the default before k_sweep_ws: one warp per replica, 10 unrolled partner
+    iterations with the bond stream interleaved (lanes = 32), 200 sweeps."""
+    _both(synth.make_inputs(4), 200, lanes=32, expect_kernel="k_sweep_group<double,32,10,")
+
+
+@pytest.mark.parametrize("config_id, kernel", [(1, "k_sweep_ws<double,1,1,"), (2, "k_sweep_ws<double,1,1,"),
+                                               (3, "k_sweep_ws<double,1,2,")])
+def test_small_configs_default_to_the_warp_specialised_kernel(config_id, kernel):
+    """Configs 1-3 (8, 32, 64 chains): the planner's default is k_sweep_ws, one pair warp and two stream warps per
+    chain; 300 sweeps here, the full runs above go through the same kernel."""
+    _both(synth.make_inputs(config_id), 300, expect_kernel=kernel)
 
 
 @pytest.mark.parametrize("lanes", [128, 256])
@@ -173,11 +188,15 @@ def _max_abs_energy(conf):
 
 # (label, N, M, E, lanes, kernel the planner must pick, sweeps, exchange_every)
 OVERLAP_CASES = [
-    ("config1_shape", 13, 8, 1, 0, "k_sweep_group<double,16,1,", 150, 10),
+    ("config1_shape", 13, 8, 1, 0, "k_sweep_ws<double,1,1,", 150, 10),
+    ("config1_shape_lanes16", 13, 8, 1, 16, "k_sweep_group<double,16,1,", 150, 10),
     ("comp_13_7_4", 100, 64, 40, 0, "k_sweep_comp<double,13,7,4,", 40, 10),
     ("comp_7_4_2", 55, 64, 40, 0, "k_sweep_comp<double,7,4,2,", 60, 10),
     ("seven_13_10_partly_filled", 100, 64, 60, 0, "k_sweep_seven<double,13,10,", 30, 10),
-    ("config4_shape", 309, 128, 1, 0, "k_sweep_group<double,32,10,", 40, 20),
+    ("config4_shape", 309, 128, 1, 0, "k_sweep_ws<double,3,4,", 40, 20),
+    ("config4_shape_lanes32", 309, 128, 1, 32, "k_sweep_group<double,32,10,", 40, 20),
+    ("ws_2_2", 100, 16, 2, 0, "k_sweep_ws<double,2,2,", 60, 10),
+    ("ws_odd_length_wrap", 37, 8, 3, 0, "k_sweep_ws<double,1,2,", 80, 7),
     ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
     ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
     ("N100_lanes32", 100, 16, 2, 32, "k_sweep_group<double,32,4,", 60, 10),
