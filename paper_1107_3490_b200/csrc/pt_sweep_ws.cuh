@@ -50,13 +50,11 @@ __device__ __forceinline__ void pt_bar_arrive(int id, int nthreads)
   asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// ring of stream records: [slot][0..3] = b0 + b2 ("accepted" left bond terms), b1 + b3 (right bond terms),
-// b4 + b6 ("rejected" left bond terms), log u;  mask = ballot of broken NEW bonds (bits 0, 1, 4)
-struct PtWsShared {
-  double rec[4][4];
-  unsigned mask[4];
-  double red[2][4];   // partial pair sums of the pair warps, double-buffered by step parity
-};
+// Ring of stream records, four deep, eight doubles each:
+//   [0] b0 + b2 ("accepted" left bond terms)   [1] b1 + b3 (right bond terms)   [2] b4 + b6 ("rejected" left)
+//   [3] log u     [4..6] the proposed position of the step's monomer (the pair warps draw no random numbers)
+// and a mask per record: the ballot of broken NEW bonds (bits 0, 1, 4).
+constexpr int kWsRec = 8;
 
 // log(v), v normal and > 0: PtNum<double>::log_ with the series by Estrin's scheme (depth 4 instead of 10), the
 // arithmetic of BondChain's levels 15..29
@@ -91,11 +89,12 @@ template <typename Real> __device__ __forceinline__ Real ws_log(Real v)
 
 // One pass of the stream for monomer m (old position xo.., proposed xn.., uniform u).  `ahead`: lanes 0 and 2
 // take the left neighbour at its proposed position, table entry + (ex, ey, ez), instead of the table entry
-// (the same separately rounded addition as the proposal itself, R7).
+// (the same separately rounded addition as the proposal itself, R7).  Returns what this lane stores
+// into the record: lanes 0, 1, 4, 5 -> entries 0, 1, 2, 3; lanes 8, 9, 10 -> the proposed position; *mask = ballot.
 template <typename Real>
-__device__ __forceinline__ void ws_stream(const PtDev& d, const PtCoords<Real>& X, int lane, int m, int N, Real xo, Real yo,
-                                          Real zo, Real xn, Real yn, Real zn, Real u, bool ahead, Real ex, Real ey,
-                                          Real ez, PtWsShared& sh, int slot)
+__device__ __forceinline__ double ws_stream(const PtDev& d, const PtCoords<Real>& X, int lane, int m, int N, Real xo, Real yo,
+                                            Real zo, Real xn, Real yn, Real zn, Real u, bool ahead, Real ex, Real ey,
+                                            Real ez, unsigned* mask)
 {
   const int role = lane;
   const int nb = (role & 1) ? m + 1 : m - 1;
@@ -121,13 +120,25 @@ __device__ __forceinline__ void ws_stream(const PtDev& d, const PtCoords<Real>& 
   const Real fc = isnew ? (Real)d.feneC : (Real)-d.feneC;   // -(K/2) R^2
   const Real bond = role != 5 ? fc * lg : (Real)0;
   const Real pairsum = bond + __shfl_xor_sync(0xffffffffu, bond, 2);
-  const unsigned mask = __ballot_sync(0xffffffffu, broke);
-  // lanes 0, 1, 4, 5 -> rec[slot][0, 1, 2, 3]; one predicated store each (a chain of ifs becomes a jump table)
-  const int idx = lane == 0 ? 0 : (lane == 1 ? 1 : (lane == 4 ? 2 : 3));
-  const bool writes = ((0x33u >> lane) & 1u) != 0u && lane < 8;
-  const double val = lane == 5 ? (double)lg : (double)pairsum;
-  if (writes) sh.rec[slot][idx] = val;
-  if (lane == 2) sh.mask[slot] = mask;
+  *mask = __ballot_sync(0xffffffffu, broke);
+  const Real pos = lane == 8 ? xn : (lane == 9 ? yn : zn);
+  return lane >= 8 ? (double)pos : (lane == 5 ? (double)lg : (double)pairsum);
+}
+// sum of n = 8, 16 or 24 numbers as a tree (depth 3, 4, 5)
+template <int n> __device__ __forceinline__ double ws_tree(double* q)
+{
+  if constexpr (n == 1) return q[0];
+  else if constexpr (n == 3) return (q[0] + q[1]) + q[2];
+  else {
+#pragma unroll
+    for (int i = 0; i < n / 2; ++i) q[i] += q[i + n / 2];
+    return ws_tree<n / 2>(q);
+  }
+}
+// entry of the record that lane `lane` stores, or -1
+__device__ __forceinline__ int ws_entry(int lane)
+{
+  return lane == 0 ? 0 : lane == 1 ? 1 : lane == 4 ? 2 : lane == 5 ? 3 : (lane >= 8 && lane < 11) ? lane - 4 : -1;
 }
 
 template <typename Real, int P, int NI, bool TRACE>
@@ -136,7 +147,9 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
 {
   static_assert(P >= 1 && P <= 3 && NI >= 1, "pair warps and partner iterations");
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ PtWsShared sh;
+  __shared__ double s_rec[4][kWsRec];     // ring of stream records
+  __shared__ unsigned s_mask[4];
+  __shared__ double s_red[2][8 * P];       // eight partial pair sums per pair warp, double-buffered by step parity
   constexpr int T = 32 * P;                               // pair threads
   constexpr int NT = 32 * (P + 2);                        // + two stream warps
   constexpr bool F2 = sizeof(Real) == 4;                  // fp32: two partners per thread and iteration
@@ -166,6 +179,7 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
     // g - 2 without waiting and waits at the barrier of step g - 1, after which its record is complete.  Two
     // barrier ids alternate with the step parity, so an arrival can never be counted for the wrong step.
     const int s = warp - P;
+    const int entry = ws_entry(lane);
     int blk_no = -1;
     DrawBlock<Real> blk;
     auto numbers = [&](int g) {   // the draw of step g (steps are asked for in increasing order)
@@ -176,9 +190,6 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       return draw_fetch<Real>(blk, g, 0u);
     };
     for (int g = s; g <= total; g += 2) {
-#ifdef PT_WS_DEBUG
-      if (blockIdx.x == 0 && lane == 0 && g < 8) printf("stream warp %d iteration %d\n", s, g);
-#endif
       if (g >= 2) pt_bar_arrive(1 + (g & 1), NT);                    // barrier of step g - 2
       Real ex = (Real)0, ey = (Real)0, ez = (Real)0;
       if (g >= 1) { const DrawBlock<Real> pv = numbers(g - 1); ex = pv.dx; ey = pv.dy; ez = pv.dz; }
@@ -186,7 +197,10 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       Real xa, ya, za;
       X.get(nx.m, xa, ya, za);
       const Real xp = PtNum<Real>::shift(xa, nx.dx), yp = PtNum<Real>::shift(ya, nx.dy), zp = PtNum<Real>::shift(za, nx.dz);
-      ws_stream<Real>(d, X, lane, nx.m, N, xa, ya, za, xp, yp, zp, nx.u, g >= 1, ex, ey, ez, sh, g & 3);
+      unsigned mask;
+      const double val = ws_stream<Real>(d, X, lane, nx.m, N, xa, ya, za, xp, yp, zp, nx.u, g >= 1, ex, ey, ez, &mask);
+      if (entry >= 0) s_rec[g & 3][entry] = val;
+      if (lane == 2) s_mask[g & 3] = mask;
       if (g < 2) {
         __syncthreads();                                            // the records of steps 0 and 1 precede the loop
         // barrier of step 0: waited for, not just arrived at -- this warp's next operation on the same id is the
@@ -203,28 +217,20 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
 
   // ---- pair warps ----
   __syncthreads();
-  DrawBlock<Real> blk = draw_block<Real>(c, false, N, width, t0, 0, lane);
-  DrawBlock<Real> nx = draw_fetch<Real>(blk, 0, 0u);
   const PtLJ<Real> lj(d);
   const double nbeta = -c.beta;
   PtNoSide noside;
   bool acc_prev = true;
-  int gstep = 0;
+  int g = 0;   // step number within the launch
   for (int sw = 0; sw < n_sweeps; ++sw) {
     const uint32_t t = t0 + (uint32_t)sw;
-    for (int k = 0; k < N; ++k) {
-      // A2: this step's numbers were fetched one step ahead
-      const DrawBlock<Real> p = nx;
-      const int g = gstep;
-      ++gstep;
-      if ((gstep & 7) == 0) blk = draw_block<Real>(c, false, N, width, t0, gstep, lane);
-      nx = draw_fetch<Real>(blk, gstep, 0u);
-      const int m = p.m;
+    for (int k = 0; k < N; ++k, ++g) {
+      // A2 comes from the stream warp: the proposed position of monomer m = k is part of the step's record
+      const int m = k;
+      const int slot = g & 3;
       Real xo, yo, zo;
       X.get(m, xo, yo, zo);
-      const Real xn = PtNum<Real>::shift(xo, p.dx);
-      const Real yn = PtNum<Real>::shift(yo, p.dy);
-      const Real zn = PtNum<Real>::shift(zo, p.dz);
+      const Real xn = (Real)s_rec[slot][4], yn = (Real)s_rec[slot][5], zn = (Real)s_rec[slot][6];
       const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
       const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
       const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
@@ -233,26 +239,21 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       Real part;
       if constexpr (F2) part = pair_groups_f2<T, NI2, 1>(lj, X, tid, m, xo, yo, zo, tdx, tdy, tdz, dd, noside);
       else part = pair_groups<Real, T, NI, 1>(lj, X, tid, m, xo, yo, zo, tdx, tdy, tdz, dd, noside);
-      // A4: warp sum, one partial per warp
-      part = group_sum<Real, 32>(part, lane, 0);
-      if (lane == 0) sh.red[g & 1][warp] = (double)part;
-#ifdef PT_WS_DEBUG
-      if (blockIdx.x == 0 && lane == 0 && g < 6) printf("pair warp %d before barrier %d\n", warp, g);
-#endif
+      // A4: two shuffle levels leave eight partial sums per warp; every decider adds all of them after the barrier
+      // (three more shuffle levels would cost ~140 cycles of the step, the loads and adds ~60)
+      part += __shfl_xor_sync(0xffffffffu, part, 16);
+      part += __shfl_xor_sync(0xffffffffu, part, 8);
+      if (lane < 8) s_red[g & 1][8 * warp + lane] = (double)part;
       pt_bar_sync(1 + (g & 1), NT);   // partial sums and the stream record of this step are complete
-#ifdef PT_WS_DEBUG
-      if (blockIdx.x == 0 && lane == 0 && g < 6) printf("pair warp %d after barrier %d\n", warp, g);
-#endif
 
-      double dEd = sh.red[g & 1][0];
-      if (P > 1) dEd += sh.red[g & 1][1];
-      if (P > 2) dEd += sh.red[g & 1][2];
-      const int slot = g & 3;
-      dEd += sh.rec[slot][1];
-      dEd += acc_prev ? sh.rec[slot][0] : sh.rec[slot][2];
-      const double logu = sh.rec[slot][3];
-      const bool bond_broken = (sh.mask[slot] & (acc_prev ? 0x03u : 0x12u)) != 0u;
-      const Real dE = (Real)dEd;
+      double q8[8 * P];
+#pragma unroll
+      for (int i = 0; i < 8 * P; ++i) q8[i] = s_red[g & 1][i];
+      const double bonds = s_rec[slot][1] + (acc_prev ? s_rec[slot][0] : s_rec[slot][2]);
+      const double logu = s_rec[slot][3];
+      const bool bond_broken = (s_mask[slot] & (acc_prev ? 0x03u : 0x12u)) != 0u;
+      const double pairs = ws_tree<8 * P>(q8);
+      const Real dE = (Real)(pairs + bonds);
 
       // A6: Metropolis, Eq. (5): accept iff dE <= 0 or u < exp(-beta dE); NaN compares false
       const bool accept = !bond_broken && (dE <= (Real)0 || logu < nbeta * (double)dE);
