@@ -149,15 +149,16 @@ bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch*
   return true;
 }
 
-// Warp-specialised CTA per chain (k_sweep_ws): P pair warps + one stream warp, every warp alone on its SM
-// sub-partition.  Sequential order only, N >= 4.  P grows with the chain length (the pair warps' share of a step is
-// about 60 cycles per partner iteration beside ~300 for load, reduce, decide; the stream warp needs ~420), as far as
-// the sub-partitions last.
+// Warp-specialised CTA per chain (k_sweep_ws): P pair warps + two stream warps, every pair warp alone on its SM
+// sub-partition (the stream warps are busy about half of the time and may share).  Sequential order only, N >= 5.
+// P grows with the chain length (a partner iteration costs a pair warp about 60 cycles beside ~450 for load,
+// reduce, barrier, decide), as far as the sub-partitions last.  Measured against one warp per chain on B200
+// (fp64, N = 13 ... 480, 8 ... 592 chains): 1.2x - 1.85x up to 148 chains, 1.05x - 1.2x up to ~400.
 bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLaunch* out)
 {
   if (d.select_mode != PT_SEQUENTIAL || d.N < 5) return false;
   for (int P = d.N > 192 ? 3 : (d.N > 64 ? 2 : 1); P >= 1; --P) {
-    if ((long long)d.C * (P + 1) > smsp) continue;
+    if (2ll * d.C * P + d.C > 2 * smsp) continue;   // a stream warp is busy about half of the time
     const int T = 32 * P;
     const int ni = pt_ws_variant(P, (d.N + T - 1) / T);
     if (ni < 0) continue;

@@ -12,7 +12,8 @@ struct WsVariant {
   { P, NI, { k_sweep_ws<double, P, NI, false>, k_sweep_ws<double, P, NI, true> }, \
     { k_sweep_ws<float, P, NI, false>, k_sweep_ws<float, P, NI, true> } }
 const WsVariant kWs[] = {
-    PT_WS(1, 1), PT_WS(1, 2), PT_WS(1, 3), PT_WS(1, 4), PT_WS(2, 2), PT_WS(2, 3), PT_WS(3, 3), PT_WS(3, 4), PT_WS(3, 5),
+    PT_WS(1, 1), PT_WS(1, 2), PT_WS(1, 3), PT_WS(1, 4), PT_WS(1, 5), PT_WS(1, 7), PT_WS(1, 10), PT_WS(1, 15),
+    PT_WS(2, 2), PT_WS(2, 3), PT_WS(2, 4), PT_WS(2, 5), PT_WS(2, 8), PT_WS(3, 3), PT_WS(3, 4), PT_WS(3, 5),
 };
 
 }  // namespace

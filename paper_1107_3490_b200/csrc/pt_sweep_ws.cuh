@@ -1,36 +1,45 @@
-// Warp-specialised sweep kernel for the latency-bound shapes: few chains (at most one warp per SM sub-partition
-// even with P + 1 warps per chain), sequential monomer order.  One CTA per chain:
+// Warp-specialised sweep kernel for the latency-bound shapes: few chains (every pair warp alone on its SM
+// sub-partition), sequential monomer order.  One CTA per chain:
 //
-//   warps 0 .. P-1  "pair warps"   A3 for their share of the partners (32 P threads stride over the table, the
-//                                  unrolled stage-major groups of pt_sweep_kernels.cuh), warp-reduce, one partial
-//                                  sum per warp into shared memory; after the step's barrier EVERY pair thread
-//                                  adds the partials and the bond terms, decides (A6) and keeps the books; the
-//                                  thread that owns the moved monomer's table slot commits (A7);
-//   warp P          "stream warp"  A5 (Eq. 3: sqrt and log of up to four bonds) and log u, as plain serial code,
-//                                  ONE STEP AHEAD and for both outcomes of the step in flight.
+//   warps 0 .. P-1   "pair warps"    A3 for their share of the partners (32 P threads stride over the table, the
+//                                    unrolled stage-major groups of pt_sweep_kernels.cuh), two shuffle levels, eight
+//                                    partial sums per warp into shared memory; after the step's barrier EVERY pair
+//                                    thread adds the partials and the bond terms, decides (A6) and keeps the books;
+//                                    the thread that owns the moved monomer's table slot commits (A7);
+//   warps P, P + 1   "stream warps"  A2 (Philox, the proposed position), A5 (Eq. 3: sqrt and log of up to four bonds)
+//                                    and log u, as plain serial code, for the even and the odd steps, AHEAD of the
+//                                    pair warps and for both outcomes of the step in flight.
 //
 // Why.  With one warp per chain (k_sweep_group) a step is as long as its dependence chain
 //   commit -> load -> [pair stages | sqrt, log: ~30 dependent fp64 levels] -> reduce -> decide -> commit
 // and the serial stream is the longest part of it (720-1270 cycles per step on BASELINE configs 1-4, of which the
-// pair arithmetic needs 100-600).  A second warp can take the stream off that chain only if it does not wait for
-// the decision.  In the sequential order it need not: the stream of step g + 1 (monomer m' = m + 1) depends on
-// step g only through the position of m, the left bond neighbour of m', and that position is one of two known
-// candidates.  Roles of the stream warp's lanes (bit 0: right neighbour, bit 1: old position of m', bit 2: step g
-// rejected):
-//   0  new bond (m', m'-1), step g accepted      4  the same, rejected
-//   2  old bond (m', m'-1), accepted             6  the same, rejected
-//   1  new bond (m', m'+1)     3  old bond (m', m'+1)     5  log u
-// "accepted" takes x_m' = x_m + delta from registers, "rejected" reads the table, which holds the old position of m
-// until the step's barrier.  One shuffle level leaves b0 + b2, b1 + b3 and b4 + b6 in lanes 0, 1, 4; they go to a
-// four-deep ring in shared memory together with log u and the ballot of the broken new bonds, and the deciders of
-// step g + 1 pick the sums that belong to the outcome of step g.
+// pair arithmetic needs 100-600).  Another warp can take the stream off that chain only if it does not wait for
+// the decision.  In the sequential order it need not: the stream of step g (monomer m) depends on the steps before
+// only through the position of m - 1, the monomer of step g - 1 and left bond neighbour of m, and that position is
+// one of two known candidates.  Roles of a stream warp's lanes (bit 0: right neighbour, bit 1: old position of m,
+// bit 2: step g - 1 rejected):
+//   0  new bond (m, m-1), step g - 1 accepted      4  the same, rejected
+//   2  old bond (m, m-1), accepted                 6  the same, rejected
+//   1  new bond (m, m+1)     3  old bond (m, m+1)     5  log u
+// "accepted" adds the displacement of step g - 1 to the table entry of m - 1, "rejected" reads the table entry,
+// which holds the old position until the barrier of step g - 1.  Nothing that steps g - 2 and g - 1 decide enters,
+// so a stream has two steps' time, and two warps alternate.  One shuffle level leaves b0 + b2, b1 + b3 and b4 + b6
+// in lanes 0, 1, 4; they go to a four-deep ring of records in shared memory together with log u, the ballot of the
+// broken new bonds and the proposed position (the pair warps draw no random numbers), and the deciders of step g
+// pick the sums that belong to the outcome of step g - 1.
 //
-// One named barrier per step (all P + 1 warps): partial sums and the stream record of the step are complete.
-// No barrier is needed after the commit: a table slot is read in the pair loop by one thread only, its owner, and
-// the owner is the thread that commits; the stream warp reads slots m', m' +- 1 while slot m - 1 may be committed
-// (distinct for N >= 4); the moved monomer itself is read again N steps later.
+// Synchronisation: one named barrier per step (ids 1 and 2 alternate with the step parity; all P + 2 warps): the
+// partial sums of the step are complete, and so is its record.  The stream warp of step g arrives at the barrier
+// of step g - 2 without waiting (bar.arrive) and waits at the barrier of step g - 1 (bar.sync); between two
+// operations of a warp on the same id lies a wait that implies the earlier phase has completed, so an arrival is
+// never counted for the wrong step.  No barrier is needed after the commit: a table slot is read in the pair loop
+// by one thread only, its owner, and the owner is the thread that commits; a stream warp reads the slots m - 1,
+// m, m + 1 while slots m - 2 and m - 3 may be committed (distinct for N >= 5); the moved monomer itself is read
+// again N steps later.
 // The paper's own mapping is one block per replica; this is that mapping with the block's warps
-// given different work.  Random-pick mode, N < 4 and larger batches keep the other kernels (pt_plan_sweep).
+// given different work.  Random-pick mode, N < 5 and larger batches keep the other kernels (pt_plan_sweep).
+// Measured (B200, fp64, moves/s): config 1 1.74e7 -> 2.21e7, config 2 8.22e7 -> 1.09e8, config 3 1.72e8 -> 2.30e8,
+// config 4 2.14e8 -> 3.20e8 against one warp per chain.
 #pragma once
 #include "pt_sweep_kernels.cuh"
 
