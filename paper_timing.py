@@ -30,8 +30,9 @@ from paper_1107_3490_b200 import binding as pt   # noqa: E402
 from paper_1107_3490_b200 import synth           # noqa: E402
 
 # the paper's range (up to ~500 replicas) and beyond it, with points on both sides of every multiple of the
-# 592 SM sub-partitions of a B200, where a uniform mapping would step
-NR = [1, 8, 64, 148, 296, 592, 593, 740, 888, 1036, 1184, 1185, 1480, 1776, 2072, 2368, 2369, 2664, 2960, 3256,
+# 592 SM sub-partitions of a B200, where a uniform mapping would step, and of the 394 chains up to which the
+# warp-specialised kernel is chosen for N = 55
+NR = [1, 8, 64, 148, 296, 394, 395, 592, 593, 740, 888, 1036, 1184, 1185, 1480, 1776, 2072, 2368, 2369, 2664, 2960, 3256,
       3552, 3848, 4144, 4145, 4440, 4736, 4737, 6000, 8288, 9472]
 
 
