@@ -78,8 +78,9 @@ typedef struct {
   int32_t nbins;       /* interior energy-histogram bins per temperature, 0 = no histogram            */
   int32_t observables; /* != 0: accumulate R_ee^2 and R_gyr^2 (Eq. 8) once per sweep                  */
   int32_t lanes;       /* threads that share one chain's Delta-E sum: 0 = choose from N and the chain
-                          count; 8, 16, 32 = that many lanes of a warp; 64, 128, 256 = one CTA of
-                          that many threads per replica                                               */
+                          count (few chains in sequential order: one CTA per chain with specialised
+                          warps, see pt_launch_info); 8, 16, 32 = that many lanes of a warp; 64, 128,
+                          256 = one CTA of that many threads per replica                              */
   double hist_emin, hist_emax;          /* histogram range, emin < emax (ignored if nbins == 0)       */
   double eps, r0, R, K, rc_over_sigma;  /* model constants; the paper's are 1, 0.7, 0.3, 40, 2.5
                                            (PAPER.md:81, :85); sigma = r0 / 2^(1/6) is derived        */
@@ -175,7 +176,10 @@ int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
  * CTA, CTAs in the grid, dynamic shared memory bytes per CTA.  Any pointer may be NULL.  With
  * lanes = 0 and between 4 and 7 chains per SM sub-partition (and N in 51..56 or 97..100) the library maps
  * 4 chains x 8 lanes + 3 chains x 10 lanes on every sub-partition; it then reports 8 lanes and 28
- * chains per CTA. */
+ * chains per CTA.  With lanes = 0, PT_SEQUENTIAL, N >= 5 and few chains (about 1.5 chains per SM
+ * sub-partition at most) every chain gets a CTA of P = 1..3 "pair" warps, which share the Delta-E sum, and
+ * two "stream" warps, which evaluate the bond terms of Eq. (3) and log u ahead of the decision; it then
+ * reports 32 P lanes and 1 chain per CTA. */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,
                    int32_t* smem_bytes);
 
