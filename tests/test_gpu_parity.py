@@ -289,6 +289,31 @@ def test_ragged_shapes(N, M, E):
         _both(inp, 40, lanes=lanes, nbins=16)
 
 
+# (N, M, E, kernel the planner must pick): the classes of the warp-specialised kernel and its limits
+WS_CASES = [
+    (5, 8, 1, "k_sweep_ws<double,1,1,"),           # the shortest chain it takes
+    (4, 8, 1, "k_sweep_group<double,"),            # below: the stream warps' table reads would meet commits
+    (64, 8, 2, "k_sweep_ws<double,1,2,"),
+    (65, 16, 1, "k_sweep_ws<double,2,2,"),
+    (200, 8, 1, "k_sweep_ws<double,3,3,"),
+    (200, 100, 3, "k_sweep_ws<double,1,7,"),       # 300 chains: one pair warp each
+    (480, 4, 1, "k_sweep_ws<double,3,5,"),
+    (55, 394, 1, "k_sweep_ws<double,1,2,"),        # the last chain count with a CTA per chain (N = 55) ...
+    (55, 395, 1, "k_sweep_group<double,32,2,"),    # ... and the first with one warp per chain
+]
+
+
+@pytest.mark.parametrize("N,M,E,kernel", WS_CASES, ids=[f"N{c[0]}_C{c[1] * c[2]}" for c in WS_CASES])
+def test_warp_specialised_classes(N, M, E, kernel):
+    """k_sweep_ws for one, two and three pair warps, short and long partner loops, chain counts up to where the planner
+    leaves it, 60 sweeps with exchanges, both instantiations (pt_sweep_ws.cuh)."""
+    T = synth.temperature_ladder(M, 0.3, 2.5)
+    reps, runs, _ = both(N, M, E, T, synth.move_halfwidths(T), synth.seeds(11, E),
+                         synth.random_walk_conformations(E, M, N, seed=7000 + N + M), 60, 10, nbins=32,
+                         label=f"ws N={N} C={M * E}", expect_kernel=kernel)
+    assert reps[False]["divergent_swaps"] == 0
+
+
 def test_zero_sweeps_and_no_exchange():
     inp = synth.make_inputs(1)
     _both(inp, 0)
