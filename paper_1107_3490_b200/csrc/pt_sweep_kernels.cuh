@@ -86,6 +86,7 @@ template <typename Real> struct BondChain {
   Real f, mp, x, e, sv, s2, z, z2, z4, z8, p01, p23, p45, p67, p89, q0, q1, pz, de;
   bool isbond, isnew, in_range;
 
+  static constexpr bool kShortChain = false;   // pair groups in the throughput form (see pair_group)
   __device__ __forceinline__ BondChain(const PtDev& dev, const PtCoords<Real>& coords) : d(dev), X(coords) {}
 
   template <int K> __device__ __forceinline__ void level()
@@ -202,28 +203,41 @@ __device__ __forceinline__ void pair_group(const PtLJ<Real>& lj, const PtCoords<
   for (int u = 0; u < CNT; ++u) X.get(s0 + (BEGIN + u) * L, bx[u], by[u], bz[u]);
 #pragma unroll
   for (int u = 0; u < CNT; ++u) { bx[u] = xo - bx[u]; by[u] = yo - by[u]; bz[u] = zo - bz[u]; }
-  PT_SIDE(0);
+  if constexpr (Side::kShortChain) {
+    // a lone warp (k_sweep_ws): the same instructions as below, as two chains of depth 3 side by side and one
+    // addition -- r_n^2 = r_o^2 + (|delta|^2 + 2 delta.b) -- instead of one chain of depth 7
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = bx[u] * bx[u];
-  PT_SIDE(1);
+    for (int u = 0; u < CNT; ++u) { ro[u] = bx[u] * bx[u]; rn[u] = fma(tdz, bz[u], dd); }
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = fma(by[u], by[u], ro[u]);
-  PT_SIDE(2);
+    for (int u = 0; u < CNT; ++u) { ro[u] = fma(by[u], by[u], ro[u]); rn[u] = fma(tdy, by[u], rn[u]); }
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) ro[u] = fma(bz[u], bz[u], ro[u]);
-  PT_SIDE(3);
+    for (int u = 0; u < CNT; ++u) { ro[u] = fma(bz[u], bz[u], ro[u]); rn[u] = fma(tdx, bx[u], rn[u]); }
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + dd;
-  PT_SIDE(4);
+    for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + rn[u];
+  } else {
+    PT_SIDE(0);
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdz, bz[u], rn[u]);
-  PT_SIDE(5);
+    for (int u = 0; u < CNT; ++u) ro[u] = bx[u] * bx[u];
+    PT_SIDE(1);
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdy, by[u], rn[u]);
-  PT_SIDE(6);
+    for (int u = 0; u < CNT; ++u) ro[u] = fma(by[u], by[u], ro[u]);
+    PT_SIDE(2);
 #pragma unroll
-  for (int u = 0; u < CNT; ++u) rn[u] = fma(tdx, bx[u], rn[u]);
-  PT_SIDE(7);
+    for (int u = 0; u < CNT; ++u) ro[u] = fma(bz[u], bz[u], ro[u]);
+    PT_SIDE(3);
+#pragma unroll
+    for (int u = 0; u < CNT; ++u) rn[u] = ro[u] + dd;
+    PT_SIDE(4);
+#pragma unroll
+    for (int u = 0; u < CNT; ++u) rn[u] = fma(tdz, bz[u], rn[u]);
+    PT_SIDE(5);
+#pragma unroll
+    for (int u = 0; u < CNT; ++u) rn[u] = fma(tdy, by[u], rn[u]);
+    PT_SIDE(6);
+#pragma unroll
+    for (int u = 0; u < CNT; ++u) rn[u] = fma(tdx, bx[u], rn[u]);
+    PT_SIDE(7);
+  }
   Real dv[2 * CNT], xv[2 * CNT], ev[2 * CNT];
 #pragma unroll
   for (int u = 0; u < CNT; ++u) {

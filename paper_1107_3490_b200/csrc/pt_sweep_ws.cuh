@@ -47,6 +47,7 @@ namespace {
 
 // the pair groups' side stream is empty here
 struct PtNoSide {
+  static constexpr bool kShortChain = true;   // pair groups in the form with the shortest dependence chain
   template <int P, int NPTS, int LEVG> __device__ __forceinline__ void run() {}
 };
 
@@ -62,8 +63,9 @@ __device__ __forceinline__ void pt_bar_arrive(int id, int nthreads)
 // Ring of stream records, four deep, eight doubles each:
 //   [0] b0 + b2 ("accepted" left bond terms)   [1] b1 + b3 (right bond terms)   [2] b4 + b6 ("rejected" left)
 //   [3] log u     [4..6] the proposed position of the step's monomer (the pair warps draw no random numbers)
+//   [7..10] 2 delta_x, 2 delta_y, 2 delta_z, |delta|^2 of the proposal (the terms of r_n^2 - r_o^2)
 // and a mask per record: the ballot of broken NEW bonds (bits 0, 1, 4).
-constexpr int kWsRec = 8;
+constexpr int kWsRec = 12;
 
 // log(v), v normal and > 0: PtNum<double>::log_ with the series by Estrin's scheme (depth 4 instead of 10), the
 // arithmetic of BondChain's levels 15..29
@@ -99,7 +101,8 @@ template <typename Real> __device__ __forceinline__ Real ws_log(Real v)
 // One pass of the stream for monomer m (old position xo.., proposed xn.., uniform u).  `ahead`: lanes 0 and 2
 // take the left neighbour at its proposed position, table entry + (ex, ey, ez), instead of the table entry
 // (the same separately rounded addition as the proposal itself, R7).  Returns what this lane stores
-// into the record: lanes 0, 1, 4, 5 -> entries 0, 1, 2, 3; lanes 8, 9, 10 -> the proposed position; *mask = ballot.
+// into the record: lanes 0, 1, 4, 5 -> entries 0, 1, 2, 3; lanes 8..14 -> the proposed position and the terms of
+// r_n^2 - r_o^2; *mask = ballot.
 template <typename Real>
 __device__ __forceinline__ double ws_stream(const PtDev& d, const PtCoords<Real>& X, int lane, int m, int N, Real xo, Real yo,
                                             Real zo, Real xn, Real yn, Real zn, Real u, bool ahead, Real ex, Real ey,
@@ -130,8 +133,19 @@ __device__ __forceinline__ double ws_stream(const PtDev& d, const PtCoords<Real>
   const Real bond = role != 5 ? fc * lg : (Real)0;
   const Real pairsum = bond + __shfl_xor_sync(0xffffffffu, bond, 2);
   *mask = __ballot_sync(0xffffffffu, broke);
-  const Real pos = lane == 8 ? xn : (lane == 9 ? yn : zn);
-  return lane >= 8 ? (double)pos : (lane == 5 ? (double)lg : (double)pairsum);
+  // what this lane stores, by selects (a nested conditional becomes a jump table)
+  const Real px = xn - xo, py = yn - yo, pz = zn - zo;   // the displacement as a pair warp would compute it
+  const Real pd = fma(pz, pz, fma(py, py, px * px));
+  Real v = pairsum;
+  v = lane == 5 ? lg : v;
+  v = lane == 8 ? xn : v;
+  v = lane == 9 ? yn : v;
+  v = lane == 10 ? zn : v;
+  v = lane == 11 ? px + px : v;
+  v = lane == 12 ? py + py : v;
+  v = lane == 13 ? pz + pz : v;
+  v = lane == 14 ? pd : v;
+  return (double)v;
 }
 // sum of n = 8, 16 or 24 numbers as a tree (depth 3, 4, 5)
 template <int n> __device__ __forceinline__ double ws_tree(double* q)
@@ -147,7 +161,13 @@ template <int n> __device__ __forceinline__ double ws_tree(double* q)
 // entry of the record that lane `lane` stores, or -1
 __device__ __forceinline__ int ws_entry(int lane)
 {
-  return lane == 0 ? 0 : lane == 1 ? 1 : lane == 4 ? 2 : lane == 5 ? 3 : (lane >= 8 && lane < 11) ? lane - 4 : -1;
+  int e = -1;
+  e = lane == 0 ? 0 : e;
+  e = lane == 1 ? 1 : e;
+  e = lane == 4 ? 2 : e;
+  e = lane == 5 ? 3 : e;
+  e = (lane >= 8 && lane < 15) ? lane - 4 : e;
+  return e;
 }
 
 template <typename Real, int P, int NI, bool TRACE>
@@ -240,9 +260,7 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       Real xo, yo, zo;
       X.get(m, xo, yo, zo);
       const Real xn = (Real)s_rec[slot][4], yn = (Real)s_rec[slot][5], zn = (Real)s_rec[slot][6];
-      const Real ex = xn - xo, ey = yn - yo, ez = zn - zo;
-      const Real dd = fma(ez, ez, fma(ey, ey, ex * ex));
-      const Real tdx = ex + ex, tdy = ey + ey, tdz = ez + ez;
+      const Real tdx = (Real)s_rec[slot][7], tdy = (Real)s_rec[slot][8], tdz = (Real)s_rec[slot][9], dd = (Real)s_rec[slot][10];
 
       // A3: this thread's partners
       Real part;
