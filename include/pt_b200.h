@@ -126,7 +126,9 @@ int pt_exchange(pt_handle* h);
 
 /* Repeats { pt_sweeps(exchange_every); pt_exchange() } until n_sweeps sweeps are done, without
  * host round trips; a last partial block of sweeps is not followed by an exchange.
- * exchange_every <= 0: no exchange at all. */
+ * exchange_every <= 0: no exchange at all.  Same results as the separate calls; where the sweep kernel is the
+ * one-CTA-per-chain kernel (see pt_launch_info) the exchange is done at the end of the sweep launch itself, by
+ * the last CTA of every ensemble to finish, instead of by a kernel of its own. */
 int pt_run(pt_handle* h, int64_t n_sweeps, int64_t exchange_every);
 
 /* Synchronises the stream and copies results to HOST arrays (NULL = skip). */

@@ -145,7 +145,7 @@ bool params_ok(const pt_params* p, std::string* why)
 
 // Device workspace layout; every array 256-byte aligned.
 struct Layout {
-  uint64_t coords, erun, tos, sot, beta, width, keys, hist, mom, obs, mcount, scount, staging,
+  uint64_t coords, erun, tos, sot, beta, width, keys, hist, mom, obs, mcount, scount, done, staging,
       e_by_temp, e_full, total;
 };
 
@@ -169,6 +169,7 @@ Layout make_layout(const pt_params* p)
   L.obs = take(C * PT_NOBS * 8);
   L.mcount = take(C * 3 * 8);
   L.scount = take(E * (M > 1 ? M - 1 : 1) * 2 * 8);
+  L.done = take(E * 4);
   L.staging = take(C * N * 3 * 8);
   L.e_by_temp = take(C * 8);
   L.e_full = take(C * 8);
@@ -264,6 +265,7 @@ int create_common(pt_handle** out, const pt_params* p, const double* T, const do
   d.obs = (double*)(base + L.obs);
   d.mcount = (unsigned long long*)(base + L.mcount);
   d.scount = (unsigned long long*)(base + L.scount);
+  d.done = (unsigned*)(base + L.done);
   h->staging = (double*)(base + L.staging);
   h->e_by_temp = (double*)(base + L.e_by_temp);
   h->e_full = (double*)(base + L.e_full);
@@ -339,6 +341,7 @@ int pt_init(pt_handle* h, const uint64_t* seeds, const double* conformations)
   for (int e = 0; e < d.E; ++e) keys[e] = make_uint2((uint32_t)(seeds[e] & 0xFFFFFFFFull), (uint32_t)(seeds[e] >> 32));
   PT_CUDA(h, cudaMemcpyAsync((void*)d.keys, keys.data(), (size_t)d.E * 8, cudaMemcpyHostToDevice, h->stream));
   PT_CUDA(h, cudaMemcpyAsync(h->staging, conformations, C * N * 3 * 8, cudaMemcpyHostToDevice, h->stream));
+  PT_CUDA(h, cudaMemsetAsync(d.done, 0, (size_t)d.E * 4, h->stream));
   PT_CUDA(h, pt_launch_scatter_init(d, h->p.precision, h->staging, h->stream));
   PT_CUDA(h, pt_launch_full_energy(d, h->p.precision, d.erun, h->stream));
   h->launches += 3;
@@ -409,10 +412,22 @@ int pt_run(pt_handle* h, int64_t n_sweeps, int64_t exchange_every)
   while (done < n_sweeps) {
     int64_t n = exchange_every;
     if (n <= 0 || n > n_sweeps - done) n = n_sweeps - done;
+    const bool exchange_follows = exchange_every > 0 && n == exchange_every;
+    // k_sweep_ws does the exchange itself at the end of the launch (the last CTA of every ensemble to finish), unless
+    // the running energies are re-based first (pt_exchange) or the sweeps need more than one launch
+    const bool rebase = ((h->x + 1) & h->x) == 0 ||
+                        (h->p.precision == PT_F32 && h->x % PT_F32_REFRESH_EVENTS == PT_F32_REFRESH_EVENTS - 1);
+    const bool fuse = exchange_follows && h->plan.kind == PT_K_WS && !rebase && n > 0 &&
+                      n <= (2147483647ll - 16) / h->d.N && h->x + 1 <= 0xFFFFFFFFll;
+    h->plan.fuse_exchange = fuse ? 1 : 0;
+    h->plan.x = (unsigned)h->x;
     int rc = pt_sweeps(h, n);
+    h->plan.fuse_exchange = 0;
     if (rc != PT_OK) return rc;
     done += n;
-    if (exchange_every > 0 && n == exchange_every) {
+    if (fuse) {
+      h->x += 1;
+    } else if (exchange_follows) {
       rc = pt_exchange(h);
       if (rc != PT_OK) return rc;
     }

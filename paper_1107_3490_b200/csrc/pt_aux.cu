@@ -81,25 +81,7 @@ __global__ void k_exchange(const PtDev d, const uint32_t x)
   const int npairs = (d.M - (int)(x & 1u)) / 2;   // pairs (i, i+1), i = parity, parity+2, ..., i+1 <= M-1
   const int tid = blockIdx.x * blockDim.x + threadIdx.x;
   if (tid >= d.E * npairs) return;
-  const int e = tid / npairs;
-  const int i = (int)(x & 1u) + 2 * (tid % npairs);
-  int* sot = d.slot_of_temp + (size_t)e * d.M;
-  int* tos = d.temp_of_slot + (size_t)e * d.M;
-  const int a = sot[i], b = sot[i + 1];
-  const double Ea = d.erun[(size_t)e * d.M + a], Eb = d.erun[(size_t)e * d.M + b];
-  const double delta = (d.beta[i] - d.beta[i + 1]) * (Ea - Eb);
-  const uint4 w = pt_draw(d.keys[e], (uint32_t)i, x, (uint32_t)e, PT_TAG_SWAP, 0u);
-  const double u = PtNum<double>::u01(w.x);
-  const bool accept = (delta >= 0.0) ? true : (u < exp(delta));
-  unsigned long long* sc = d.scount + ((size_t)e * (d.M - 1) + i) * 2;
-  sc[0] += 1ull;
-  if (accept) {
-    sc[1] += 1ull;
-    sot[i] = b; sot[i + 1] = a;
-    tos[a] = i + 1; tos[b] = i;
-  }
-  if (d.tr_swap && (long long)x < d.cap_events)
-    d.tr_swap[((size_t)e * d.cap_events + x) * (size_t)(d.M - 1) + i] = accept ? 2 : 1;
+  pt_exchange_pair(d, tid / npairs, (int)(x & 1u) + 2 * (tid % npairs), x);
 }
 
 // Read-out in temperature order: energies and AoS fp64 conformations.

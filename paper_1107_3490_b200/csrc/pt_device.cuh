@@ -205,6 +205,30 @@ template <> struct PtNum<float> {
 //            = u (A u - B) - C,   u = 1/r^6,  A = 4 eps sigma^12,  B = 4 eps sigma^6,  C = E_LJ(r_c)
 // The sums accumulate u (A u - B) with u = 0 for the pairs outside the cutoff, and count the pairs
 // inside; the caller subtracts C * count once per sum.
+// Section 3.3, Eq. (6): the swap test of the neighbour pair (i, i + 1) of ensemble e at exchange
+// event x.  The temperature labels of the two slots are swapped; coordinates stay where they are.  Called by
+// k_exchange (one thread per pair) and by the last CTA of an ensemble in k_sweep_ws (fused exchange).
+__device__ __forceinline__ void pt_exchange_pair(const PtDev& d, int e, int i, uint32_t x)
+{
+  int* sot = d.slot_of_temp + (size_t)e * d.M;
+  int* tos = d.temp_of_slot + (size_t)e * d.M;
+  const int a = sot[i], b = sot[i + 1];
+  const double Ea = d.erun[(size_t)e * d.M + a], Eb = d.erun[(size_t)e * d.M + b];
+  const double delta = (d.beta[i] - d.beta[i + 1]) * (Ea - Eb);
+  const uint4 w = pt_draw(d.keys[e], (uint32_t)i, x, (uint32_t)e, PT_TAG_SWAP, 0u);
+  const double u = PtNum<double>::u01(w.x);
+  const bool accept = (delta >= 0.0) ? true : (u < exp(delta));
+  unsigned long long* sc = d.scount + ((size_t)e * (d.M - 1) + i) * 2;
+  sc[0] += 1ull;
+  if (accept) {
+    sc[1] += 1ull;
+    sot[i] = b; sot[i + 1] = a;
+    tos[a] = i + 1; tos[b] = i;
+  }
+  if (d.tr_swap && (long long)x < d.cap_events)
+    d.tr_swap[((size_t)e * d.cap_events + x) * (size_t)(d.M - 1) + i] = accept ? 2 : 1;
+}
+
 template <typename Real> struct PtLJ {
   Real A, nB, C, rc2, c, mhc;   // c = B / A = sigma^-6, mhc = -c / 2
   __device__ __forceinline__ explicit PtLJ(const PtDev& d)

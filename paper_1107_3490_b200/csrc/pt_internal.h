@@ -42,6 +42,7 @@ struct PtDev {
   double* obs;                 // [C][PT_NOBS]
   unsigned long long* mcount;  // [C][3]
   unsigned long long* scount;  // [E][max(M-1,1)][2]
+  unsigned* done;              // [E] chains of the ensemble that have finished the launch (fused exchange, k_sweep_ws)
   // trace (test support), temperature-indexed
   unsigned char* tr_move;
   unsigned char* tr_swap;
@@ -72,6 +73,10 @@ struct PtLaunch {
   int wcount[8];       // chains of warp w (<= 32 / lanes; the other chain slots stay idle)
   int woff[8];         // shared-memory offset of warp w's first chain, in Reals
   int wdelay[8];       // start delay of warp w in cycles
+  // k_sweep_ws, set per launch by pt_run: the exchange event that follows the sweeps is done by the last CTA of
+  // every ensemble to finish (no exchange kernel, no launch gap)
+  int fuse_exchange;   // 0 = none
+  unsigned x;          // index of that exchange event
 };
 
 enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4, PT_K_WS = 5 };

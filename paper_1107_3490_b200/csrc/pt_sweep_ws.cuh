@@ -310,6 +310,30 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
   else __syncwarp();
   for (int j = tid; j < N; j += T) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
   if (tid == 0) ctx_store(d, c, n_sweeps);
+
+  // B1 fused (pt_run): the exchange event that follows these sweeps is done by the CTA that is the last of its
+  // ensemble to finish -- no exchange kernel and no launch gap, which are 4 us of an interval of 45 us on config 1.
+  // Each CTA publishes its chain's running energy (fence), then counts itself; the one that counts M - 1 others
+  // sees all of them and swaps the labels of its ensemble's neighbour pairs (Eq. 6), one thread per pair.
+  if (pl.fuse_exchange) {
+    __shared__ int s_last;
+    __threadfence();
+    if (P > 1) pt_bar_sync(3, T);
+    else __syncwarp();
+    if (tid == 0) {
+      const unsigned before = atomicAdd(&d.done[c.e], 1u);
+      s_last = before == (unsigned)(d.M - 1);
+      if (s_last) d.done[c.e] = 0u;   // everyone of this ensemble has counted: ready for the next launch
+    }
+    if (P > 1) pt_bar_sync(3, T);
+    else __syncwarp();
+    if (s_last) {
+      __threadfence();
+      const uint32_t x = pl.x;
+      const int npairs = (d.M - (int)(x & 1u)) / 2;
+      for (int q = tid; q < npairs; q += T) pt_exchange_pair(d, c.e, (int)(x & 1u) + 2 * q, x);
+    }
+  }
 }
 
 }  // namespace
