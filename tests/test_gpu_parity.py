@@ -314,6 +314,20 @@ def test_warp_specialised_classes(N, M, E, kernel):
     assert reps[False]["divergent_swaps"] == 0
 
 
+@pytest.mark.parametrize("N,M,E,S", [(20, 5, 3, 3), (37, 8, 2, 1), (100, 7, 2, 4)])
+def test_fused_exchange_equals_separate_calls(N, M, E, S):
+    """Under pt_run the warp-specialised kernel does the exchange event at the end of the sweep launch (the last CTA of
+    every ensemble to finish); pt_sweeps + pt_exchange called one by one use the exchange kernel.  Both against the
+    oracle: odd and even numbers of temperatures, several ensembles, exchange after every S sweeps (the events before
+    which E_run is re-based, 0, 1, 3, 7, ..., take the separate path in both)."""
+    T = synth.temperature_ladder(M, 0.3, 2.5)
+    args = (N, M, E, T, synth.move_halfwidths(T), synth.seeds(13, E), synth.random_walk_conformations(E, M, N, seed=8100 + N))
+    for stepwise in (False, True):
+        reps, runs, _ = both(*args, 40 * S, S, nbins=32, stepwise=stepwise, label=f"fused exchange N={N} M={M} stepwise={stepwise}",
+                             expect_kernel="k_sweep_ws<double,")
+        assert reps[False]["divergent_swaps"] == 0 and runs[False][0]["counters"] == (40 * S, 40)
+
+
 def test_zero_sweeps_and_no_exchange():
     inp = synth.make_inputs(1)
     _both(inp, 0)
