@@ -435,9 +435,13 @@ def run_ours(args, rank, world, local):
             "energies": ((wl.E, wl.M), torch.float64),
             "moments": ((wl.E, wl.M, 3), torch.float64),
             "conformations": ((wl.E, wl.M, wl.N, 3), torch.float64)}.items()}
-        hist = np.zeros((wl.E, wl.M, wl.nbins + 2), dtype=np.uint64)
-        mc = np.zeros((wl.E, wl.M, 3), dtype=np.uint64)
-        sc = np.zeros((wl.E, max(wl.M - 1, 1), 2), dtype=np.uint64)
+        # the integer outputs as well (the histograms are 93 % of the bytes that come back): pinned int64 storage,
+        # viewed as the uint64 the ABI writes
+        def pinned_u64(shape):
+            return torch.zeros(shape, dtype=torch.int64).pin_memory().numpy().view(np.uint64)
+        hist = pinned_u64((wl.E, wl.M, wl.nbins + 2))
+        mc = pinned_u64((wl.E, wl.M, 3))
+        sc = pinned_u64((wl.E, max(wl.M - 1, 1), 2))
         h2d = conf_h.nbytes + inp.seeds.nbytes
         d2h = sum(a.nbytes for a in outs.values()) + hist.nbytes + mc.nbytes + (sc.nbytes if wl.M > 1 else 0)
 
