@@ -178,9 +178,9 @@ int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
  * CTA, CTAs in the grid, dynamic shared memory bytes per CTA.  Any pointer may be NULL.  With
  * lanes = 0 and between 4 and 7 chains per SM sub-partition (and N in 51..56 or 97..100) the library maps
  * 4 chains x 8 lanes + 3 chains x 10 lanes on every sub-partition; it then reports 8 lanes and 28
- * chains per CTA.  With lanes = 0, PT_SEQUENTIAL, N >= 5 and few chains (about 1.5 chains per SM
+ * chains per CTA.  With lanes = 0, PT_SEQUENTIAL, N >= 6 and few chains (about 1.5 chains per SM
  * sub-partition at most) every chain gets a CTA of P = 1..3 "pair" warps, which share the Delta-E sum, and
- * two "stream" warps, which evaluate the bond terms of Eq. (3) and log u ahead of the decision; it then
+ * two or three "stream" warps, which evaluate the bond terms of Eq. (3) and log u ahead of the decision; it then
  * reports 32 P lanes and 1 chain per CTA. */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,
                    int32_t* smem_bytes);

@@ -156,7 +156,7 @@ bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch*
 // (fp64, N = 13 ... 480, 8 ... 592 chains): 1.2x - 1.85x up to 148 chains, 1.05x - 1.2x up to ~400.
 bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLaunch* out)
 {
-  if (d.select_mode != PT_SEQUENTIAL || d.N < 5) return false;
+  if (d.select_mode != PT_SEQUENTIAL || d.N < 6) return false;   // three stream warps read m - 1 .. m + 1 beside commits of m - 4 .. m - 2
   for (int P = d.N > 192 ? 3 : (d.N > 64 ? 2 : 1); P >= 1; --P) {
     if (2ll * d.C * P + d.C > 2 * smsp) continue;   // a stream warp is busy about half of the time
     const int T = 32 * P;
@@ -168,7 +168,7 @@ bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLa
     pl.ni = ni;
     pl.Ns = table_slots(T, ni, real_bytes);
     pl.sstride = 3 * pl.Ns;
-    pl.threads = 32 * (P + 2);
+    pl.threads = 32 * (P + pt_ws_stream_warps(P, ni));
     pl.chains_per_cta = 1;
     pl.grid = d.C;
     pl.smem_bytes = pl.sstride * real_bytes;

@@ -6,9 +6,10 @@
 //                                    partial sums per warp into shared memory; after the step's barrier EVERY pair
 //                                    thread adds the partials and the bond terms, decides (A6) and keeps the books;
 //                                    the thread that owns the moved monomer's table slot commits (A7);
-//   warps P, P + 1   "stream warps"  A2 (Philox, the proposed position), A5 (Eq. 3: sqrt and log of up to four bonds)
-//                                    and log u, as plain serial code, for the even and the odd steps, AHEAD of the
-//                                    pair warps and for both outcomes of the step in flight.
+//   warps P .. P+SW-1 "stream warps" A2 (Philox, the proposed position), A5 (Eq. 3: sqrt and log of up to four bonds)
+//                                    and log u, as plain serial code, warp P + s for the steps g = s (mod SW), AHEAD of
+//                                    the pair warps and for both outcomes of the step in flight.  SW = 2, or 3 where one
+//                                    pair warp with a short partner loop is faster than two streams can feed it.
 //
 // Why.  With one warp per chain (k_sweep_group) a step is as long as its dependence chain
 //   commit -> load -> [pair stages | sqrt, log: ~30 dependent fp64 levels] -> reduce -> decide -> commit
@@ -22,24 +23,24 @@
 //   2  old bond (m, m-1), accepted                 6  the same, rejected
 //   1  new bond (m, m+1)     3  old bond (m, m+1)     5  log u
 // "accepted" adds the displacement of step g - 1 to the table entry of m - 1, "rejected" reads the table entry,
-// which holds the old position until the barrier of step g - 1.  Nothing that steps g - 2 and g - 1 decide enters,
-// so a stream has two steps' time, and two warps alternate.  One shuffle level leaves b0 + b2, b1 + b3 and b4 + b6
-// in lanes 0, 1, 4; they go to a four-deep ring of records in shared memory together with log u, the ballot of the
+// which holds the old position until the barrier of step g - 1.  Nothing that the steps before g - 1 decide enters,
+// so a stream has SW steps' time, and SW warps take turns.  One shuffle level leaves b0 + b2, b1 + b3 and b4 + b6
+// in lanes 0, 1, 4; they go to a ring of eight records in shared memory together with log u, the ballot of the
 // broken new bonds and the proposed position (the pair warps draw no random numbers), and the deciders of step g
 // pick the sums that belong to the outcome of step g - 1.
 //
-// Synchronisation: one named barrier per step (ids 1 and 2 alternate with the step parity; all P + 2 warps): the
-// partial sums of the step are complete, and so is its record.  The stream warp of step g arrives at the barrier
-// of step g - 2 without waiting (bar.arrive) and waits at the barrier of step g - 1 (bar.sync); between two
-// operations of a warp on the same id lies a wait that implies the earlier phase has completed, so an arrival is
-// never counted for the wrong step.  No barrier is needed after the commit: a table slot is read in the pair loop
+// Synchronisation: one named barrier per step (ids 1 .. SW in turn; all P + SW warps): the partial sums of the step
+// are complete, and so is its record.  The stream warp of step g arrives at the barriers of the steps g - SW .. g - 2
+// without waiting (bar.arrive) and waits at the barrier of step g - 1 (bar.sync); between two operations of a warp
+// on the same id lies a wait that implies the earlier phase has completed, so an arrival is never counted for the
+// wrong step.  No barrier is needed after the commit: a table slot is read in the pair loop
 // by one thread only, its owner, and the owner is the thread that commits; a stream warp reads the slots m - 1,
-// m, m + 1 while slots m - 2 and m - 3 may be committed (distinct for N >= 5); the moved monomer itself is read
-// again N steps later.
+// m, m + 1 while slots m - 2 .. m - SW - 1 may be committed (distinct for N >= 6); the moved monomer itself is
+// read again N steps later.
 // The paper's own mapping is one block per replica; this is that mapping with the block's warps
-// given different work.  Random-pick mode, N < 5 and larger batches keep the other kernels (pt_plan_sweep).
-// Measured (B200, fp64, moves/s): config 1 1.74e7 -> 2.29e7, config 2 8.22e7 -> 1.12e8, config 3 1.72e8 -> 2.40e8,
-// config 4 2.14e8 -> 3.23e8 against one warp per chain.
+// given different work.  Random-pick mode, N < 6 and larger batches keep the other kernels (pt_plan_sweep).
+// Measured (B200, fp64, moves/s): config 1 1.74e7 -> 2.5e7, config 2 8.22e7 -> 1.23e8, config 3 1.72e8 -> 2.58e8,
+// config 4 2.14e8 -> 3.2e8 against one warp per chain.
 #pragma once
 #include "pt_sweep_kernels.cuh"
 
@@ -170,17 +171,20 @@ __device__ __forceinline__ int ws_entry(int lane)
   return e;
 }
 
-template <typename Real, int P, int NI, bool TRACE>
-__global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, const PtLaunch pl, const uint32_t t0,
+// SW: stream warps (2 or 3); warp P + s takes the steps g = s (mod SW) and has SW steps' time for each.
+template <typename Real, int P, int NI, bool TRACE, int SW>
+__global__ void __launch_bounds__(32 * (P + SW), 1) k_sweep_ws(const PtDev d, const PtLaunch pl, const uint32_t t0,
                                                            const int n_sweeps)
 {
   static_assert(P >= 1 && P <= 3 && NI >= 1, "pair warps and partner iterations");
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ double s_rec[4][kWsRec];     // ring of stream records
-  __shared__ unsigned s_mask[4];
+  constexpr int RING = 8;                  // records in flight: written up to SW steps ahead, read for one step
+  __shared__ double s_rec[RING][kWsRec];  // ring of stream records
+  __shared__ unsigned s_mask[RING];
   __shared__ double s_red[2][8 * P];       // eight partial pair sums per pair warp, double-buffered by step parity
   constexpr int T = 32 * P;                               // pair threads
-  constexpr int NT = 32 * (P + 2);                        // + two stream warps
+  constexpr int NT = 32 * (P + SW);                       // + the stream warps
+  static_assert(SW == 2 || SW == 3, "stream warps");
   constexpr bool F2 = sizeof(Real) == 4;                  // fp32: two partners per thread and iteration
   constexpr int NI2 = (NI + 1) / 2;
   constexpr int Ns = F2 ? 2 * T * NI2 : T * NI;
@@ -202,11 +206,11 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
   __syncthreads();
 
   if (warp >= P) {
-    // ---- stream warps: warp P takes the even steps, warp P + 1 the odd ones ----
-    // The stream of step g needs nothing that steps g - 2 and g - 1 decide (only the two candidates for the left
-    // neighbour, the monomer of step g - 1), so it has two steps' time: the warp arrives at the barrier of step
-    // g - 2 without waiting and waits at the barrier of step g - 1, after which its record is complete.  Two
-    // barrier ids alternate with the step parity, so an arrival can never be counted for the wrong step.
+    // ---- stream warps: warp P + s takes the steps g = s (mod SW) ----
+    // The stream of step g needs nothing that the steps before g - 1 decide (only the two candidates for the left
+    // neighbour, the monomer of step g - 1), so it has SW steps' time: the warp arrives at the barriers of the steps
+    // g - SW .. g - 2 without waiting and waits at the barrier of step g - 1, after which its record is complete.
+    // SW barrier ids take turns, so an arrival can never be counted for the wrong step.
     const int s = warp - P;
     const int entry = ws_entry(lane);
     int blk_no = -1;
@@ -218,8 +222,11 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       }
       return draw_fetch<Real>(blk, g, 0u);
     };
-    for (int g = s; g <= total; g += 2) {
-      if (g >= 2) pt_bar_arrive(1 + (g & 1), NT);                    // barrier of step g - 2
+    for (int g = s; g <= total; g += SW) {
+      if (g >= SW) {                                                 // barriers of the steps g - SW .. g - 2
+#pragma unroll
+        for (int j = SW; j >= 2; --j) pt_bar_arrive(1 + (g - j) % SW, NT);
+      }
       Real ex = (Real)0, ey = (Real)0, ez = (Real)0;
       if (g >= 1) { const DrawBlock<Real> pv = numbers(g - 1); ex = pv.dx; ey = pv.dy; ez = pv.dz; }
       const DrawBlock<Real> nx = numbers(g);
@@ -228,19 +235,21 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       const Real xp = PtNum<Real>::shift(xa, nx.dx), yp = PtNum<Real>::shift(ya, nx.dy), zp = PtNum<Real>::shift(za, nx.dz);
       unsigned mask;
       const double val = ws_stream<Real>(d, X, lane, nx.m, N, xa, ya, za, xp, yp, zp, nx.u, g >= 1, ex, ey, ez, &mask);
-      if (entry >= 0) s_rec[g & 3][entry] = val;
-      if (lane == 2) s_mask[g & 3] = mask;
-      if (g < 2) {
-        __syncthreads();                                            // the records of steps 0 and 1 precede the loop
-        // barrier of step 0: waited for, not just arrived at -- this warp's next operation on the same id is the
-        // wait of step 2, and an arrival must never be counted for an earlier step than it is meant for
-        if (g == 1) pt_bar_sync(1, NT);
+      if (entry >= 0) s_rec[g & (RING - 1)][entry] = val;
+      if (lane == 2) s_mask[g & (RING - 1)] = mask;
+      if (g < SW) {
+        __syncthreads();                                            // the records of the first SW steps precede the loop
+        // the barriers of the steps before g: arrived at, the last one waited for -- between two operations of a warp
+        // on one id there must be a wait that implies the earlier phase is complete, or an arrival is counted for the
+        // wrong step
+        for (int b = 0; b + 1 < g; ++b) pt_bar_arrive(1 + b % SW, NT);
+        if (g >= 1) pt_bar_sync(1 + (g - 1) % SW, NT);
       } else {
-        pt_bar_sync(1 + ((g - 1) & 1), NT);                         // barrier of step g - 1
+        pt_bar_sync(1 + (g - 1) % SW, NT);                          // barrier of step g - 1
       }
     }
-    // the loop ends with g = total or total - 1; in the second case the barrier of the last step is still owed
-    if ((((total - s) & ~1) + s) == total - 1) pt_bar_arrive(1 + ((total - 1) & 1), NT);
+    // the loop ends with some g in total - SW + 1 .. total; the barriers of the steps from there on are still owed
+    for (int b = total - (total - s) % SW; b < total; ++b) pt_bar_arrive(1 + b % SW, NT);
     return;
   }
 
@@ -256,7 +265,7 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
     for (int k = 0; k < N; ++k, ++g) {
       // A2 comes from the stream warp: the proposed position of monomer m = k is part of the step's record
       const int m = k;
-      const int slot = g & 3;
+      const int slot = g & (RING - 1);
       Real xo, yo, zo;
       X.get(m, xo, yo, zo);
       const Real xn = (Real)s_rec[slot][4], yn = (Real)s_rec[slot][5], zn = (Real)s_rec[slot][6];
@@ -271,7 +280,7 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
       part += __shfl_xor_sync(0xffffffffu, part, 16);
       part += __shfl_xor_sync(0xffffffffu, part, 8);
       if (lane < 8) s_red[g & 1][8 * warp + lane] = (double)part;
-      pt_bar_sync(1 + (g & 1), NT);   // partial sums and the stream record of this step are complete
+      pt_bar_sync(1 + g % SW, NT);   // partial sums and the stream record of this step are complete
 
       double q8[8 * P];
 #pragma unroll
@@ -299,14 +308,14 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
     }
 
     // A8: measurement once per sweep; the last commit may have come from another pair warp
-    if (P > 1) pt_bar_sync(3, T);
+    if (P > 1) pt_bar_sync(SW + 1, T);
     else __syncwarp();
     if (d.observables && warp == 0) measure_shape<Real, 32>(d, c, N, lane, 0, X);
     if (tid == 0) measure_energy(d, c, t);
   }
 
   // A9: shared memory -> HBM
-  if (P > 1) pt_bar_sync(3, T);
+  if (P > 1) pt_bar_sync(SW + 1, T);
   else __syncwarp();
   for (int j = tid; j < N; j += T) X.get(j, gx[j], gx[d.Ng + j], gx[2 * d.Ng + j]);
   if (tid == 0) ctx_store(d, c, n_sweeps);
@@ -318,14 +327,14 @@ __global__ void __launch_bounds__(32 * (P + 2), 1) k_sweep_ws(const PtDev d, con
   if (pl.fuse_exchange) {
     __shared__ int s_last;
     __threadfence();
-    if (P > 1) pt_bar_sync(3, T);
+    if (P > 1) pt_bar_sync(SW + 1, T);
     else __syncwarp();
     if (tid == 0) {
       const unsigned before = atomicAdd(&d.done[c.e], 1u);
       s_last = before == (unsigned)(d.M - 1);
       if (s_last) d.done[c.e] = 0u;   // everyone of this ensemble has counted: ready for the next launch
     }
-    if (P > 1) pt_bar_sync(3, T);
+    if (P > 1) pt_bar_sync(SW + 1, T);
     else __syncwarp();
     if (s_last) {
       __threadfence();

@@ -291,8 +291,8 @@ def test_ragged_shapes(N, M, E):
 
 # (N, M, E, kernel the planner must pick): the classes of the warp-specialised kernel and its limits
 WS_CASES = [
-    (5, 8, 1, "k_sweep_ws<double,1,1,"),           # the shortest chain it takes
-    (4, 8, 1, "k_sweep_group<double,"),            # below: the stream warps' table reads would meet commits
+    (6, 8, 1, "k_sweep_ws<double,1,1,"),           # the shortest chain it takes
+    (5, 8, 1, "k_sweep_group<double,"),            # below: the stream warps' table reads would meet commits
     (64, 8, 2, "k_sweep_ws<double,1,2,"),
     (65, 16, 1, "k_sweep_ws<double,2,2,"),
     (200, 8, 1, "k_sweep_ws<double,3,3,"),
