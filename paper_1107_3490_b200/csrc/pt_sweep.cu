@@ -152,12 +152,15 @@ bool plan_comp(const PtDev& d, int precision, int real_bytes, int sms, PtLaunch*
 // Warp-specialised CTA per chain (k_sweep_ws): P pair warps + two stream warps, every pair warp alone on its SM
 // sub-partition (the stream warps are busy about half of the time and may share).  Sequential order only, N >= 5.
 // P grows with the chain length (a partner iteration costs a pair warp about 60 cycles beside ~450 for load,
-// reduce, barrier, decide), as far as the sub-partitions last.  Measured against one warp per chain on B200
+// reduce, barrier, decide; every further pair warp adds eight partial sums and a barrier participant), as far as
+// the sub-partitions last.  Measured against one warp per chain on B200
 // (fp64, N = 13 ... 480, 8 ... 592 chains): 1.2x - 1.85x up to 148 chains, 1.05x - 1.2x up to ~400.
 bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLaunch* out)
 {
   if (d.select_mode != PT_SEQUENTIAL || d.N < 6) return false;   // three stream warps read m - 1 .. m + 1 beside commits of m - 4 .. m - 2
-  for (int P = d.N > 192 ? 3 : (d.N > 64 ? 2 : 1); P >= 1; --P) {
+  // measured on B200 (fp64, us per step at 128 chains): one pair warp 0.25 - 0.29 up to N = 128, two 0.30 - 0.36 up to
+  // N = 320 (three there: 0.36 - 0.40), three 0.43 beyond (two: 0.47)
+  for (int P = d.N > 320 ? 3 : (d.N > 128 ? 2 : 1); P >= 1; --P) {
     if (2ll * d.C * P + d.C > 2 * smsp) continue;   // a stream warp is busy about half of the time
     const int T = 32 * P;
     const int ni = pt_ws_variant(P, (d.N + T - 1) / T);

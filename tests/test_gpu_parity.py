@@ -66,10 +66,10 @@ def test_config3_full_run():
 
 
 def test_config4_full_run():
-    """N=309, M=128, all 2000 sweeps, default mapping: one CTA per replica, three pair warps (4 partner iterations
+    """N=309, M=128, all 2000 sweeps, default mapping: one CTA per replica, two pair warps (5 partner iterations
     each) and two stream warps (k_sweep_ws)."""
-    rep, g, _ = _both(synth.make_inputs(4), 2000, nbins=4096, expect_kernel="k_sweep_ws<double,3,4,")
-    assert g[0]["launch_info"]["lanes"] == 96 and g[0]["counters"] == (2000, 100)
+    rep, g, _ = _both(synth.make_inputs(4), 2000, nbins=4096, expect_kernel="k_sweep_ws<double,2,5,")
+    assert g[0]["launch_info"]["lanes"] == 64 and g[0]["counters"] == (2000, 100)
 
 
 def test_config4_one_warp_per_replica():
@@ -193,9 +193,10 @@ OVERLAP_CASES = [
     ("comp_13_7_4", 100, 64, 40, 0, "k_sweep_comp<double,13,7,4,", 40, 10),
     ("comp_7_4_2", 55, 64, 40, 0, "k_sweep_comp<double,7,4,2,", 60, 10),
     ("seven_13_10_partly_filled", 100, 64, 60, 0, "k_sweep_seven<double,13,10,", 30, 10),
-    ("config4_shape", 309, 128, 1, 0, "k_sweep_ws<double,3,4,", 40, 20),
+    ("config4_shape", 309, 128, 1, 0, "k_sweep_ws<double,2,5,", 40, 20),
+    ("ws_three_pair_warps", 400, 8, 1, 0, "k_sweep_ws<double,3,5,", 30, 10),
     ("config4_shape_lanes32", 309, 128, 1, 32, "k_sweep_group<double,32,10,", 40, 20),
-    ("ws_2_2", 100, 16, 2, 0, "k_sweep_ws<double,2,2,", 60, 10),
+    ("ws_1_4", 100, 16, 2, 0, "k_sweep_ws<double,1,4,", 60, 10),
     ("ws_odd_length_wrap", 37, 8, 3, 0, "k_sweep_ws<double,1,2,", 80, 7),
     ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
     ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
@@ -294,8 +295,10 @@ WS_CASES = [
     (6, 8, 1, "k_sweep_ws<double,1,1,"),           # the shortest chain it takes
     (5, 8, 1, "k_sweep_group<double,"),            # below: the stream warps' table reads would meet commits
     (64, 8, 2, "k_sweep_ws<double,1,2,"),
-    (65, 16, 1, "k_sweep_ws<double,2,2,"),
-    (200, 8, 1, "k_sweep_ws<double,3,3,"),
+    (65, 16, 1, "k_sweep_ws<double,1,3,"),
+    (129, 16, 1, "k_sweep_ws<double,2,3,"),
+    (200, 8, 1, "k_sweep_ws<double,2,4,"),
+    (330, 6, 1, "k_sweep_ws<double,3,4,"),
     (200, 100, 3, "k_sweep_ws<double,1,7,"),       # 300 chains: one pair warp each
     (480, 4, 1, "k_sweep_ws<double,3,5,"),
     (55, 394, 1, "k_sweep_ws<double,1,2,"),        # the last chain count with a CTA per chain (N = 55) ...
