@@ -40,7 +40,7 @@
 // The paper's own mapping is one block per replica; this is that mapping with the block's warps
 // given different work.  Random-pick mode, N < 6 and larger batches keep the other kernels (pt_plan_sweep).
 // Measured (B200, fp64, moves/s): config 1 1.74e7 -> 2.5e7, config 2 8.22e7 -> 1.23e8, config 3 1.72e8 -> 2.58e8,
-// config 4 2.14e8 -> 3.2e8 against one warp per chain.
+// config 4 2.14e8 -> 3.5e8 against one warp per chain.
 #pragma once
 #include "pt_sweep_kernels.cuh"
 
