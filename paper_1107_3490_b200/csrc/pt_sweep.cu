@@ -159,7 +159,7 @@ bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLa
 {
   if (d.select_mode != PT_SEQUENTIAL || d.N < 6) return false;   // three stream warps read m - 1 .. m + 1 beside commits of m - 4 .. m - 2
   // measured on B200 (fp64, us per step at 128 chains): one pair warp 0.25 - 0.29 up to N = 128, two 0.30 - 0.36 up to
-  // N = 320 (three there: 0.36 - 0.40), three 0.43 beyond (two: 0.47)
+  // N = 320 (three there: 0.36 - 0.40), three 0.43 beyond (two: 0.47); N = 481 ... 1920: 0.49 - 0.93 (k_sweep_cta: 0.98 - 1.65)
   for (int P = d.N > 320 ? 3 : (d.N > 128 ? 2 : 1); P >= 1; --P) {
     if (2ll * d.C * P + d.C > 2 * smsp) continue;   // a stream warp is busy about half of the time
     const int T = 32 * P;

@@ -18,7 +18,7 @@ const WsVariant kWs[] = {
     PT_WS(1, 1, 3), PT_WS(1, 2, 3), PT_WS(1, 3, 3), PT_WS(1, 4, 3), PT_WS(1, 5, 3), PT_WS(1, 7, 3),
     PT_WS(1, 10, 2), PT_WS(1, 15, 2),
     PT_WS(2, 3, 2), PT_WS(2, 4, 2), PT_WS(2, 5, 2), PT_WS(2, 8, 2),
-    PT_WS(3, 4, 2), PT_WS(3, 5, 2),
+    PT_WS(3, 4, 2), PT_WS(3, 5, 2), PT_WS(3, 7, 2), PT_WS(3, 10, 2), PT_WS(3, 15, 2), PT_WS(3, 20, 2),
 };
 
 }  // namespace

@@ -301,6 +301,8 @@ WS_CASES = [
     (330, 6, 1, "k_sweep_ws<double,3,4,"),
     (200, 100, 3, "k_sweep_ws<double,1,7,"),       # 300 chains: one pair warp each
     (480, 4, 1, "k_sweep_ws<double,3,5,"),
+    (600, 4, 1, "k_sweep_ws<double,3,7,"),         # beyond the unrolled one-warp kernels: before, one CTA per replica
+    (1000, 2, 1, "k_sweep_ws<double,3,15,"),
     (55, 394, 1, "k_sweep_ws<double,1,2,"),        # the last chain count with a CTA per chain (N = 55) ...
     (55, 395, 1, "k_sweep_group<double,32,2,"),    # ... and the first with one warp per chain
 ]
