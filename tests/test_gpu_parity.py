@@ -333,6 +333,21 @@ def test_fused_exchange_equals_separate_calls(N, M, E, S):
         assert reps[False]["divergent_swaps"] == 0 and runs[False][0]["counters"] == (40 * S, 40)
 
 
+@pytest.mark.parametrize("N,M,E,n,S", [(30, 32, 1, 40000, 10), (40, 16, 8, 10000, 7), (150, 12, 2, 3000, 5)])
+def test_warp_specialised_long_runs(N, M, E, n, S):
+    """Long untraced runs of k_sweep_ws (one, one and two pair warps; 3.8e7, 5.1e7, 1.1e7 decisions; thousands of fused
+    exchange events): a rare ordering fault between pair warps, stream warps and the committing thread would surface as
+    one divergent decision, and every later coordinate would differ.  Final coordinates bitwise, counters, histograms."""
+    T = synth.temperature_ladder(M, 0.3, 3.0)
+    args = (N, M, E, T, synth.move_halfwidths(T), synth.seeds(21, E), synth.random_walk_conformations(E, M, N, seed=N + M), n, S)
+    g, _ = run_gpu(*args, trace_sweeps=0, recompute=False)
+    o, _ = run_oracle(*args, trace_sweeps=0)
+    assert g["kernel"].startswith("k_sweep_ws<double,") and g["kernel"].endswith("trace=0>"), g["kernel"]
+    assert np.array_equal(g["conformations"].view(np.uint64), o["conformations"].view(np.uint64))
+    assert np.array_equal(g["move_counts"], o["move_counts"]) and np.array_equal(g["swap_counts"], o["swap_counts"])
+    assert np.array_equal(g["histograms"], o["histograms"])
+
+
 def test_zero_sweeps_and_no_exchange():
     inp = synth.make_inputs(1)
     _both(inp, 0)
