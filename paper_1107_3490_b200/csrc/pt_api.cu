@@ -417,7 +417,7 @@ int pt_run(pt_handle* h, int64_t n_sweeps, int64_t exchange_every)
     // the running energies are re-based first (pt_exchange) or the sweeps need more than one launch
     const bool rebase = ((h->x + 1) & h->x) == 0 ||
                         (h->p.precision == PT_F32 && h->x % PT_F32_REFRESH_EVENTS == PT_F32_REFRESH_EVENTS - 1);
-    const bool fuse = exchange_follows && h->plan.kind == PT_K_WS && !rebase && n > 0 &&
+    const bool fuse = exchange_follows && (h->plan.kind == PT_K_WS || h->plan.kind == PT_K_WSG) && !rebase && n > 0 &&
                       n <= (2147483647ll - 16) / h->d.N && h->x + 1 <= 0xFFFFFFFFll;
     h->plan.fuse_exchange = fuse ? 1 : 0;
     h->plan.x = (unsigned)h->x;

@@ -79,13 +79,15 @@ struct PtLaunch {
   unsigned x;          // index of that exchange event
 };
 
-enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4, PT_K_WS = 5 };
+enum { PT_K_GROUP = 0, PT_K_COMP = 1, PT_K_CTA = 2, PT_K_SEVEN = 3, PT_K_SEVEN_FULL = 4, PT_K_WS = 5, PT_K_WSG = 6 };
 
 // Kernel tables, one per translation unit that instantiates sweep kernels (nullptr = not in this unit).
 PtSweepFn pt_lookup_group(int lanes, int ni, int precision, bool trace);   // pt_sweep_group.cu
 PtSweepFn pt_lookup_ws(int pair_warps, int ni, int precision, bool trace);   // pt_sweep_ws.cu
 int pt_ws_variant(int pair_warps, int ni_needed);
-int pt_ws_stream_warps(int pair_warps, int ni);                           // stream warps of that instantiation (2 or 3)                          // smallest instantiated NI >= ni_needed, or -1
+int pt_ws_stream_warps(int pair_warps, int ni);
+PtSweepFn pt_lookup_wsg(int chains_per_cta, int ni, int precision, bool trace);   // pt_sweep_wsg.cu
+int pt_wsg_variant(int chains_per_cta, int ni_needed);                           // stream warps of that instantiation (2 or 3)                          // smallest instantiated NI >= ni_needed, or -1
 PtSweepFn pt_lookup_cta(int precision, bool trace);                        // pt_sweep_group.cu
 PtSweepFn pt_lookup_comp(int kind, const int nik[4], int precision, bool trace);   // pt_sweep_comp*.cu
 // the unrolled variants of k_sweep_group: smallest NI >= ni_needed for this lane count, 0 = run-time loop

@@ -57,6 +57,7 @@ PtSweepFn kernel_of(const PtLaunch& pl, int precision, bool trace)
 {
   if (pl.kind == PT_K_CTA) return pt_lookup_cta(precision, trace);
   if (pl.kind == PT_K_WS) return pt_lookup_ws(pl.lanes / 32, pl.ni, precision, trace);
+  if (pl.kind == PT_K_WSG) return pt_lookup_wsg(pl.chains_per_cta, pl.ni, precision, trace);
   if (pl.kind == PT_K_COMP || pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
     return pt_lookup_comp(pl.kind, pl.nik, precision, trace);
   return pt_lookup_group(pl.lanes, pl.ni, precision, trace);
@@ -182,6 +183,28 @@ bool plan_ws(const PtDev& d, int precision, int real_bytes, long long smsp, PtLa
   return false;
 }
 
+// Several chains per CTA with shared stream warps (k_sweep_wsg): G = 4 chains, one pair warp each, three stream warps.
+bool plan_wsg(const PtDev& d, int precision, int real_bytes, PtLaunch* out)
+{
+  if (d.select_mode != PT_SEQUENTIAL || d.N < 6) return false;
+  const int G = 4;
+  const int ni = pt_wsg_variant(G, (d.N + 31) / 32);
+  if (ni < 0) return false;
+  PtLaunch pl{};
+  pl.kind = PT_K_WSG;
+  pl.lanes = 32;
+  pl.ni = ni;
+  pl.Ns = table_slots(32, ni, real_bytes);
+  pl.sstride = 3 * pl.Ns;
+  pl.threads = 32 * (G + 3);
+  pl.chains_per_cta = G;
+  pl.grid = (d.C + G - 1) / G;
+  pl.smem_bytes = G * pl.sstride * real_bytes;
+  if (!kernel_of(pl, precision, false)) return false;
+  *out = pl;
+  return true;
+}
+
 }  // namespace
 
 cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, PtLaunch* plan)
@@ -203,9 +226,15 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
   if (L == 0) {
     // More chains than SM sub-partitions: composed CTAs, chains spread evenly over the SMs (no staircase in
     // the number of replicas beyond the one of the most loaded sub-partition).
-    if ((long long)d.C > smsp) done = plan_comp(d, precision, real_bytes, sms, &pl);
+    // Short chains in batches just beyond the range of a CTA per chain: four chains per CTA with shared stream warps
+    // (measured, B200 fp64, us per step: N <= 64 at 395 ... 592 chains 0.31 - 0.32 against 0.375 - 0.385 with one warp per
+    // chain; N <= 32 at 593 ... 1184 chains 0.39 against 0.43 - 0.44 composed; longer chains and larger batches lose)
+    const int ni32 = (d.N + 31) / 32;
+    if ((long long)d.C > smsp && (long long)d.C <= 2 * smsp && ni32 == 1) done = plan_wsg(d, precision, real_bytes, &pl);
+    if (!done && (long long)d.C > smsp) done = plan_comp(d, precision, real_bytes, sms, &pl);
     // Few chains: a step is as long as its dependence chain; a second warp takes the bond stream off it.
     if (!done) done = plan_ws(d, precision, real_bytes, smsp, &pl);
+    if (!done && (long long)d.C <= smsp && ni32 <= 2) done = plan_wsg(d, precision, real_bytes, &pl);
     if (!done) {
       // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
       // loop) that still leave every warp alone on its SM sub-partition; a second warp on a
@@ -273,6 +302,7 @@ void pt_sweep_kernel_desc(const PtLaunch& pl, int precision, bool trace, char* b
 {
   const char* real = precision == PT_F32 ? "float" : "double";
   if (pl.kind == PT_K_CTA) snprintf(buf, n, "k_sweep_cta<%s,threads=%d,trace=%d>", real, pl.threads, trace ? 1 : 0);
+  else if (pl.kind == PT_K_WSG) snprintf(buf, n, "k_sweep_wsg<%s,%d,chains=%d,trace=%d>", real, pl.ni, pl.chains_per_cta, trace ? 1 : 0);
   else if (pl.kind == PT_K_WS) snprintf(buf, n, "k_sweep_ws<%s,%d,%d,trace=%d>", real, pl.lanes / 32, pl.ni, trace ? 1 : 0);
   else if (pl.kind == PT_K_SEVEN || pl.kind == PT_K_SEVEN_FULL)
     snprintf(buf, n, "k_sweep_seven<%s,%d,%d,%s,trace=%d>", real, pl.nik[0], pl.nik[3],

@@ -139,7 +139,7 @@ def test_mixed_mapping_at_the_papers_chain_length():
 # ---- variants and edge cases ----------------------------------------------------------------
 
 # (N, chains) -> chains per CTA and the sub-partition loads the planner must produce on 148 SMs
-COMPOSED = [(30, 600, 5), (55, 4144, 28), (30, 1336, 10), (30, 2000, 14), (30, 2960, 20), (30, 3400, 23), (30, 3848, 26),
+COMPOSED = [(40, 600, 5), (55, 4144, 28), (30, 1336, 10), (30, 2000, 14), (30, 2960, 20), (30, 3400, 23), (30, 3848, 26),
             (30, 4440, 30), (30, 4736, 32), (30, 5000, 17), (17, 1200, 9), (64, 2400, 17), (80, 3000, 21),
             (104, 1480, 10), (128, 1000, 7), (100, 2376, 17)]
 
@@ -198,6 +198,7 @@ OVERLAP_CASES = [
     ("config4_shape_lanes32", 309, 128, 1, 32, "k_sweep_group<double,32,10,", 40, 20),
     ("ws_1_4", 100, 16, 2, 0, "k_sweep_ws<double,1,4,", 60, 10),
     ("ws_odd_length_wrap", 37, 8, 3, 0, "k_sweep_ws<double,1,2,", 80, 7),
+    ("wsg_four_chains_per_cta", 37, 8, 60, 0, "k_sweep_wsg<double,2,chains=4,", 40, 7),
     ("N100_lanes8", 100, 16, 2, 8, "k_sweep_group<double,8,13,", 60, 10),
     ("N100_lanes16", 100, 16, 2, 16, "k_sweep_group<double,16,7,", 60, 10),
     ("N100_lanes32", 100, 16, 2, 32, "k_sweep_group<double,32,4,", 60, 10),
@@ -304,7 +305,12 @@ WS_CASES = [
     (600, 4, 1, "k_sweep_ws<double,3,7,"),         # beyond the unrolled one-warp kernels: before, one CTA per replica
     (1000, 2, 1, "k_sweep_ws<double,3,15,"),
     (55, 394, 1, "k_sweep_ws<double,1,2,"),        # the last chain count with a CTA per chain (N = 55) ...
-    (55, 395, 1, "k_sweep_group<double,32,2,"),    # ... and the first with one warp per chain
+    (55, 395, 1, "k_sweep_wsg<double,2,chains=4,"),   # ... beyond: four chains per CTA share the stream warps (397: a partly filled CTA)
+    (55, 397, 1, "k_sweep_wsg<double,2,chains=4,"),
+    (20, 5, 100, "k_sweep_wsg<double,1,chains=4,"),    # the chains of a CTA belong to different ensembles; fused exchange
+    (30, 148, 5, "k_sweep_wsg<double,1,chains=4,"),    # 740 chains: two such CTAs per SM
+    (55, 593, 1, "k_sweep_comp<double,7,4,2,"),        # N > 32 beyond 592 chains: composed CTAs
+    (100, 500, 1, "k_sweep_group<double,32,4,"),       # N > 64 between 395 and 592 chains: one warp per chain
 ]
 
 
@@ -333,7 +339,7 @@ def test_fused_exchange_equals_separate_calls(N, M, E, S):
         assert reps[False]["divergent_swaps"] == 0 and runs[False][0]["counters"] == (40 * S, 40)
 
 
-@pytest.mark.parametrize("N,M,E,n,S", [(30, 32, 1, 40000, 10), (40, 16, 8, 10000, 7), (150, 12, 2, 3000, 5)])
+@pytest.mark.parametrize("N,M,E,n,S", [(30, 32, 1, 40000, 10), (40, 16, 8, 10000, 7), (150, 12, 2, 3000, 5), (24, 8, 60, 3000, 5)])
 def test_warp_specialised_long_runs(N, M, E, n, S):
     """Long untraced runs of k_sweep_ws (one, one and two pair warps; 3.8e7, 5.1e7, 1.1e7 decisions; thousands of fused
     exchange events): a rare ordering fault between pair warps, stream warps and the committing thread would surface as
@@ -342,7 +348,7 @@ def test_warp_specialised_long_runs(N, M, E, n, S):
     args = (N, M, E, T, synth.move_halfwidths(T), synth.seeds(21, E), synth.random_walk_conformations(E, M, N, seed=N + M), n, S)
     g, _ = run_gpu(*args, trace_sweeps=0, recompute=False)
     o, _ = run_oracle(*args, trace_sweeps=0)
-    assert g["kernel"].startswith("k_sweep_ws<double,") and g["kernel"].endswith("trace=0>"), g["kernel"]
+    assert g["kernel"].startswith(("k_sweep_ws<double,", "k_sweep_wsg<double,")) and g["kernel"].endswith("trace=0>"), g["kernel"]
     assert np.array_equal(g["conformations"].view(np.uint64), o["conformations"].view(np.uint64))
     assert np.array_equal(g["move_counts"], o["move_counts"]) and np.array_equal(g["swap_counts"], o["swap_counts"])
     assert np.array_equal(g["histograms"], o["histograms"])
