@@ -181,7 +181,8 @@ int pt_set_counters(pt_handle* h, int64_t t_sweeps, int64_t x_events);
  * chains per CTA.  With lanes = 0, PT_SEQUENTIAL, N >= 6 and few chains (about 1.5 chains per SM
  * sub-partition at most) every chain gets a CTA of P = 1..3 "pair" warps, which share the Delta-E sum, and
  * two or three "stream" warps, which evaluate the bond terms of Eq. (3) and log u ahead of the decision; it then
- * reports 32 P lanes and 1 chain per CTA. */
+ * reports 32 P lanes and 1 chain per CTA (short chains in somewhat larger batches: 32 lanes, 4 chains per CTA, the
+ * stream warps shared). */
 int pt_launch_info(const pt_handle* h, int32_t* lanes, int32_t* chains_per_cta, int32_t* grid,
                    int32_t* smem_bytes);
 
