@@ -228,13 +228,14 @@ cudaError_t pt_plan_sweep(const PtDev& d, int precision, int lanes_requested, Pt
     // the number of replicas beyond the one of the most loaded sub-partition).
     // Short chains in batches just beyond the range of a CTA per chain: four chains per CTA with shared stream warps
     // (measured, B200 fp64, us per step: N <= 64 at 395 ... 592 chains 0.31 - 0.32 against 0.375 - 0.385 with one warp per
-    // chain; N <= 32 at 593 ... 1184 chains 0.39 against 0.43 - 0.44 composed; longer chains and larger batches lose)
+    // chain, N = 100 0.397 against 0.408; N <= 32 at 593 ... 1184 chains 0.39 against 0.43 - 0.44 composed; longer chains
+    // and larger batches lose; two chains per CTA never beat k_sweep_ws)
     const int ni32 = (d.N + 31) / 32;
     if ((long long)d.C > smsp && (long long)d.C <= 2 * smsp && ni32 == 1) done = plan_wsg(d, precision, real_bytes, &pl);
     if (!done && (long long)d.C > smsp) done = plan_comp(d, precision, real_bytes, sms, &pl);
     // Few chains: a step is as long as its dependence chain; a second warp takes the bond stream off it.
     if (!done) done = plan_ws(d, precision, real_bytes, smsp, &pl);
-    if (!done && (long long)d.C <= smsp && ni32 <= 2) done = plan_wsg(d, precision, real_bytes, &pl);
+    if (!done && (long long)d.C <= smsp && ni32 <= 4) done = plan_wsg(d, precision, real_bytes, &pl);
     if (!done) {
       // Few very long chains: one CTA per replica.  Otherwise the most lanes per chain (shortest partner
       // loop) that still leave every warp alone on its SM sub-partition; a second warp on a

@@ -12,7 +12,7 @@ struct WsgVariant {
   { G, NI, { k_sweep_wsg<double, NI, false, G>, k_sweep_wsg<double, NI, true, G> },      \
     { k_sweep_wsg<float, NI, false, G>, k_sweep_wsg<float, NI, true, G> } }
 const WsgVariant kWsg[] = {
-    PT_WSG(4, 1), PT_WSG(4, 2),
+    PT_WSG(4, 1), PT_WSG(4, 2), PT_WSG(4, 3), PT_WSG(4, 4),
 };
 
 }  // namespace

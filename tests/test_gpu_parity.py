@@ -310,7 +310,8 @@ WS_CASES = [
     (20, 5, 100, "k_sweep_wsg<double,1,chains=4,"),    # the chains of a CTA belong to different ensembles; fused exchange
     (30, 148, 5, "k_sweep_wsg<double,1,chains=4,"),    # 740 chains: two such CTAs per SM
     (55, 593, 1, "k_sweep_comp<double,7,4,2,"),        # N > 32 beyond 592 chains: composed CTAs
-    (100, 500, 1, "k_sweep_group<double,32,4,"),       # N > 64 between 395 and 592 chains: one warp per chain
+    (100, 500, 1, "k_sweep_wsg<double,4,chains=4,"),   # up to N = 128 between 395 and 592 chains
+    (150, 500, 1, "k_sweep_group<double,32,7,"),       # longer chains there: one warp per chain
 ]
 
 
