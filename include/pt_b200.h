@@ -203,6 +203,25 @@ const char* pt_last_error(const pt_handle* h);
  * sum of Eq. 5 is plain FMA-pipe work, no tensor cores).  tflops HOST. */
 int pt_fma_peak(int precision, int iters, int reps, void* cuda_stream, double* tflops);
 
+/* ---- the one entry point that allocates nothing ------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the full energy of Eq. (4) of n_chains conformations, the quantity pt_recompute_energy returns,
+ * computed with scratch that lives in a static device array of the library instead of a workspace.
+ *   p                  model constants and N (eps, r0, R, K, rc_over_sigma, N are read; the rest is ignored)
+ *   dev_conformations  DEVICE pointer, [n_chains][N][3] fp64 (x, y, z of monomer 0, 1, ...), read only
+ *   dev_energies       DEVICE pointer, [n_chains] fp64, written
+ *   stream             a cudaStream_t (NULL = default stream); the call only enqueues, it does not synchronise
+ * The current device is used.  No cudaMalloc, cudaFree or allocating library call is made; the first call on a device
+ * asks for the scratch array's address (cudaGetSymbolAddress).  n_chains > PT_NOALLOC_MAX_CHAINS is PT_EINVAL: split
+ * the batch.  Every GPU that loads the library holds the array (576 KiB) until the process exits.  All calls share
+ * it: calls that overlap on the GPU (two streams, two host threads) race -- serialise them.  Energies agree with
+ * pt_recompute_energy up to the order of summation (~1e-15 relative).  Errors: PT_EINVAL, PT_ECUDA; the message is
+ * pt_noalloc_last_error() (per host thread). */
+#define PT_NOALLOC_MAX_CHAINS 8192
+int pt_energy_noalloc(const pt_params* p, const double* dev_conformations, double* dev_energies, int64_t n_chains,
+                      void* stream);
+const char* pt_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

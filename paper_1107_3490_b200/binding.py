@@ -26,7 +26,7 @@ SYMBOLS = ("pt_workspace_bytes", "pt_create", "pt_create_with_workspace", "pt_de
            "pt_sweeps", "pt_exchange", "pt_run", "pt_read", "pt_recompute_energy", "pt_reset_stats",
            "pt_set_trace", "pt_counters", "pt_set_counters", "pt_launch_info", "pt_sweep_kernel_name",
            "pt_kernel_launches", "pt_last_error",
-           "pt_fma_peak")
+           "pt_fma_peak", "pt_energy_noalloc", "pt_noalloc_last_error")
 
 
 class PtParams(C.Structure):
@@ -105,6 +105,23 @@ def _ptr(a, ct):
 def _check(h, rc):
     if rc != PT_OK:
         msg = lib().pt_last_error(h)
+        raise PtError(rc, msg.decode() if msg else "")
+
+
+PT_NOALLOC_MAX_CHAINS = 8192
+
+
+def pt_energy_noalloc(params: PtParams, dev_conformations, dev_energies, n_chains: int, stream=None):
+    """pt_energy_noalloc of include/pt_b200.h: torch CUDA tensors (fp64, contiguous) in and out, nothing allocated."""
+    L = lib()
+    L.pt_energy_noalloc.argtypes = [C.POINTER(PtParams), C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+    L.pt_energy_noalloc.restype = C.c_int
+    L.pt_noalloc_last_error.restype = C.c_char_p
+    rc = L.pt_energy_noalloc(C.byref(params), C.c_void_p(dev_conformations.data_ptr() if dev_conformations is not None else 0),
+                             C.c_void_p(dev_energies.data_ptr() if dev_energies is not None else 0), int(n_chains),
+                             C.c_void_p(stream.cuda_stream if stream is not None else 0))
+    if rc != PT_OK:
+        msg = L.pt_noalloc_last_error()
         raise PtError(rc, msg.decode() if msg else "")
 
 

@@ -19,7 +19,7 @@ CSRC = PKG / "csrc"
 LIB = PKG / "libpt_b200.so"
 OBJ = PKG / "build"
 # the sweep kernels are instantiated in several translation units so that they compile in parallel
-SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu", "pt_sweep_group.cu", "pt_sweep_ws.cu", "pt_sweep_wsg.cu"] + \
+SOURCES = ["pt_api.cu", "pt_aux.cu", "pt_sweep.cu", "pt_peak.cu", "pt_sweep_group.cu", "pt_sweep_ws.cu", "pt_sweep_wsg.cu", "pt_noalloc.cu"] + \
           [f"pt_sweep_comp{u}.cu" for u in range(8)]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
